@@ -1,0 +1,352 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the Arnold-web hot path on B200 (metric: BASELINE.json).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config 3] [--order 4] [--horizon STEPS] [--no-e2e] [--no-cpu-baseline]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input:
+aw_init_shell (a1) -> aw_integrate over the config's full horizon (a2 + a3 + a4, chained launches)
+-> aw_indicator FLI image (a5) -> aw_density histogram (a6) [-> NCCL all-reduce of the histogram, N > 1].
+Workload at N = 1: BASELINE.json configs[3] (2048 x 2048 scan, eps = 3e-2, dt = 0.005, 2e5 steps, FLI),
+the configuration the metric's target is quoted on.  Under torchrun (N > 1) every rank scans its own
+2048 x 2048 strip of a 2048 x (2048 N) image of the same action square (weak scaling; no data-path
+collective except the histogram sum).
+
+value   = live trajectory-steps / s, whole job, inputs resident in HBM (device-timed, max over ranks)
+e2e     = same metric through aw_map_host: host (pinned) state in, image + histogram out, copies timed
+roofline= fp64 ALU bound: nominal flops (498 / traj-step for order 4 with tangent) per
+          integrate launch / its CUDA-event duration, against 148 SM x 64 DFMA/clk x 2 x 1.965 GHz
+cpu_baseline = the oracle (oracle/aw_oracle.cpp, as it stands) on the host cores, bounded sample
+--impl reference = the oracle as the reference arm (rank 0 only).
+"""
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "trajectory-steps/s (fp64, with tangent map)"
+UNIT = "traj-steps/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--order", type=int, default=0, help="0 = the config's (4); 6 = the paper's scheme")
+    ap.add_argument("--horizon", type=int, default=0, help="integration steps per pass (0 = the config's)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------- clocks
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def start(self):
+        if self.nv:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thread:
+            self._thread.join()
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+# ------------------------------------------------------------------------------------------- oracle arm
+
+def oracle_rate(cfg, order, tangent, seconds, rank_rows=None):
+    """Time the oracle, as it stands, on all host cores on a bounded sample of the workload:
+    a sub-lattice of the config's grid (same eps, dt, stride, order, tangent), for a prefix of the horizon
+    sized to ~`seconds` of wall time.  Returns (traj-steps/s, cores, description)."""
+    import numpy as np
+    import oracle
+    oracle.build()
+    cores = os.cpu_count() or 1
+    sub = 64                                     # 64 x 64 = 4096-trajectory sub-lattice of the grid
+    st = oracle.State(sub * sub, tangent=tangent, wind=True)
+    st.order = order
+    g = oracle.make_grid(sub, sub, cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"], cfg["cx"],
+                         cfg["cy"], cfg["r"])
+    oracle.init_shell(st, g, cfg["E"], cfg["eps"], cfg["seed"])
+    live = int((st.status == 1).sum())
+
+    def run(steps):
+        edges = np.linspace(0, st.n, cores + 1).astype(int)
+        ts = [threading.Thread(target=oracle.integrate, args=(st, steps, cfg["dt"], cfg["stride"]),
+                               kwargs=dict(k0=int(a), k1=int(b), advance_clock=False))
+              for a, b in zip(edges[:-1], edges[1:]) if b > a]
+        t0 = time.perf_counter()
+        [t.start() for t in ts]
+        [t.join() for t in ts]
+        return time.perf_counter() - t0
+
+    dt_cal = run(cfg["stride"] * 2)                                   # calibration: 200 steps
+    rate_cal = live * cfg["stride"] * 2 / max(dt_cal, 1e-6)
+    steps = int(seconds * rate_cal / live) // cfg["stride"] * cfg["stride"]
+    steps = max(cfg["stride"], min(steps, cfg["steps"]))
+    el = run(steps)
+    desc = ("%dx%d sub-lattice of the %dx%d grid (%d live), first %d of %d steps, order %d, tangent=%s, "
+            "stride %d, %d threads over disjoint trajectory ranges"
+            % (sub, sub, cfg["gx"], cfg["gy"], live, steps, cfg["steps"], order, tangent, cfg["stride"], cores))
+    return live * steps / el, cores, desc, live * steps, el
+
+
+def run_reference(args, cfg, order, tangent):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    per = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_rate(cfg, order, tangent, min(per, 2.0))
+    vals, work, el = [], 0, 0.0
+    desc, cores = "", 0
+    for _ in range(args.steps):
+        v, cores, desc, w, e = oracle_rate(cfg, order, tangent, per)
+        vals.append(v)
+        work += w
+        el += e
+    value = work / el
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / max(1, args.steps),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "gpu_launches": 0,
+            "config": {"workload": cfg["name"], "order": order, "tangent": tangent, "dt": cfg["dt"],
+                       "eps": cfg["eps"], "stride": cfg["stride"], "sample": desc},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------- our arm
+
+def run_ours(args, cfg, order, tangent):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_1107_4107_b200 import build as awbuild
+    awbuild.build()
+    import paper_1107_4107_b200 as aw
+    from paper_1107_4107_b200 import parallel
+    from paper_1107_4107_b200.configs import (FP64_PEAK_TFLOPS_NOMINAL, HIST_G, HIST_HI, HIST_LO,
+                                               NOMINAL_FLOPS)
+
+    gx, gy = cfg["gx"], cfg["gy"]
+    n = gx * gy
+    horizon = args.horizon or cfg["steps"]
+    horizon = max(cfg["stride"], horizon // cfg["stride"] * cfg["stride"])
+    lo_y, hi_y = parallel.strip_bounds(cfg["lo"], cfg["hi"], world, rank)   # rank's strip of the image
+    grid = aw.make_grid(gx, gy, cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"], cfg["cx"], cfg["cy"],
+                        cfg["r"], 1, 0, lo_y=lo_y, hi_y=hi_y)
+    ens = aw.Ensemble(n, tangent=tangent, wind=True, order=order, device=dev)
+    image = torch.empty(n, dtype=torch.float64, device=dev)
+    hist = torch.zeros((HIST_G, HIST_G), dtype=torch.int32, device=dev)
+    dropped = torch.zeros(1, dtype=torch.int64, device=dev)
+    stream = torch.cuda.current_stream()
+    kind = aw.AW_IND_FLI if tangent else aw.AW_IND_DH
+
+    integ_events = []
+
+    def one_pass(record):
+        aw.aw_init_shell(ens, grid, cfg["E"], cfg["eps"], cfg["seed"])
+        hist.zero_()
+        dropped.zero_()
+        if record:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+        aw.aw_integrate(ens, n, horizon, cfg["dt"], cfg["stride"])
+        if record:
+            e1.record(stream)
+            integ_events.append((e0, e1))
+        aw.aw_indicator(ens, kind, 0.0, out=image)
+        aw.aw_density(ens, hist, HIST_LO, HIST_HI, 0, dropped)
+        if world > 1:
+            parallel.allreduce_hist(hist)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        one_pass(False)
+    barrier()
+    live = int((ens.status[:n] == 1).sum().item())
+    clocks = ClockSampler(local)
+    launches0 = aw.aw_launch_count()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    clocks.start()
+    t0.record(stream)
+    for _ in range(args.steps):
+        one_pass(True)
+    t1.record(stream)
+    barrier()
+    clk = clocks.stop()
+    launches = aw.aw_launch_count() - launches0
+    ms = torch.tensor([t0.elapsed_time(t1)], dtype=torch.float64, device=dev)
+    livet = torch.tensor([live], dtype=torch.int64, device=dev)
+    if world > 1:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        dist.all_reduce(livet, op=dist.ReduceOp.SUM)
+    total_ms = ms.item()
+    live_all = int(livet.item())
+    value = live_all * horizon * args.steps / (total_ms * 1e-3)
+
+    # dominant kernel: integrate_kernel — average launch duration from CUDA events on its stream
+    integ_ms = sum(a.elapsed_time(b) for a, b in integ_events)
+    n_integ_launches = args.steps * math.ceil(horizon / (20000 // cfg["stride"] * cfg["stride"]))
+    flops_per_step = NOMINAL_FLOPS[(order, tangent)]
+    launch_ms = integ_ms / n_integ_launches
+    steps_per_launch = horizon * args.steps / n_integ_launches
+    achieved = live * steps_per_launch * flops_per_step / (launch_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "integrate_kernel<%d,%s>" % (3 if order == 4 else 7, str(tangent).lower()),
+                "achieved": achieved, "peak": FP64_PEAK_TFLOPS_NOMINAL, "unit": "TFLOP/s",
+                "frac": achieved / FP64_PEAK_TFLOPS_NOMINAL, "traffic": None,
+                "peak_source": "derived: 148 SM x 64 DFMA/clk/SM x 2 flop x 1.965 GHz (DESIGN.md §8); "
+                               "MEASURED_PEAKS.json has no fp64 entry",
+                "flops_per_traj_step_nominal": flops_per_step,
+                "launch_ms": launch_ms, "launches_timed": n_integ_launches,
+                "kernel_share_of_step": integ_ms / total_ms}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "grid": [gx, gy], "trajectories_per_gpu": n,
+                       "live_trajectories": live_all, "eps": cfg["eps"], "E": cfg["E"], "dt": cfg["dt"],
+                       "steps_per_pass": horizon, "stride": cfg["stride"], "order": order,
+                       "tangent": tangent, "outputs": "FLI image fp64 + 1024x1024 uint32 density",
+                       "parallelism": "dp%d (one image strip per rank)" % world,
+                       "l2": "state planes %.0f MB per pass > 126 MB L2 (no flush needed)"
+                             % (n * (16 * 8 + 12 + 1) / 1e6)},
+            "clocks": clk, "gpu_launches": int(launches), "roofline": roofline}
+
+    # measured DFMA peak beside the derived one (rank 0; independent chains, all SMs)
+    if rank == 0:
+        try:
+            sms = torch.cuda.get_device_properties(dev).multi_processor_count
+            best = 0.0
+            for chains in (8, 16):
+                msd, cnt = aw.aw_dfma_peak_probe(sms * 8, 256, chains, 1 << 16, device=dev)
+                best = max(best, 2.0 * cnt / (msd * 1e-3) / 1e12)
+            roofline["peak_measured_dfma_tflops"] = best
+            roofline["frac_of_measured_dfma"] = achieved / best
+        except Exception as e:  # the probe is evidence, not the product
+            roofline["peak_measured_dfma_tflops"] = None
+            roofline["peak_probe_error"] = str(e)
+
+    # e2e: host (pinned) state -> aw_map_host -> image + histogram on the host, copies inside the timing
+    if not args.no_e2e:
+        aw.aw_init_shell(ens, grid, cfg["E"], cfg["eps"], cfg["seed"])
+        torch.cuda.synchronize()
+        host_in = dict(q=ens.q.cpu().pin_memory(), acc=ens.acc.cpu().pin_memory(),
+                       wind=ens.wind.cpu().pin_memory(), status=ens.status[:n].cpu().pin_memory())
+        if tangent:
+            host_in["w"] = ens.w.cpu().pin_memory()
+        out = dict(image=torch.empty(n, dtype=torch.float64).pin_memory(),
+                   hist=torch.empty((HIST_G, HIST_G), dtype=torch.int32).pin_memory(),
+                   dropped=torch.zeros(1, dtype=torch.int64).pin_memory())
+        hist_dev = torch.empty(HIST_G * HIST_G + 2, dtype=torch.int32, device=dev)
+        h2d = sum(t.numel() * t.element_size() for t in host_in.values())
+        d2h = sum(t.numel() * t.element_size() for t in out.values())
+        # warm the path once with a short horizon, then time one full pass per rank
+        aw.aw_map_host(ens, host_in, cfg["stride"], cfg["dt"], cfg["stride"], kind, 0.0, (HIST_G, HIST_G),
+                       HIST_LO, HIST_HI, image, hist_dev, out)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        w0 = time.perf_counter()
+        e0.record(stream)
+        aw.aw_map_host(ens, host_in, horizon, cfg["dt"], cfg["stride"], kind, 0.0, (HIST_G, HIST_G),
+                       HIST_LO, HIST_HI, image, hist_dev, out)
+        if world > 1:
+            parallel.allreduce_hist(hist_dev[:HIST_G * HIST_G])
+        e1.record(stream)
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - w0
+        ems = torch.tensor([max(e0.elapsed_time(e1), wall * 1e3)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(ems, op=dist.ReduceOp.MAX)
+        line["e2e"] = {"value": live_all * horizon / (ems.item() * 1e-3), "unit": UNIT,
+                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                       "ms": ems.item(), "api": "aw_map_host (pinned host state in; FLI image + histogram out)"}
+
+    if rank == 0 and not args.no_cpu_baseline and world == 1:
+        v, cores, desc, _, _ = oracle_rate(cfg, order, tangent, args.cpu_seconds)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    from paper_1107_4107_b200.configs import CONFIGS
+    cfg = dict(CONFIGS[args.config])
+    order = args.order or cfg["order"]
+    tangent = cfg["tangent"]
+    if args.impl == "reference":
+        run_reference(args, cfg, order, tangent)
+    else:
+        run_ours(args, cfg, order, tangent)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,204 @@
+/* aw.h — C ABI of libaw: the ensemble hot path of arXiv 1107.4107 ("Mapping the Arnold web with a
+ * GPU-supercomputer") as hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * Citations: P:<n> = line n of the paper text; R<n> = reading n in DESIGN.md §3;
+ * §8(x) = SURVEY.md hot-path scope table.
+ *
+ * What the library computes:
+ *   model      H(P,X) = P^2/2 + eps * H_p(X)                       P:33 eq.(1)
+ *              H_p(x,y,z) = cos x cos y (1 + cos 2z)                P:43 eq.(2)
+ *   scheme     fixed-step symplectic composition (Yoshida 1990)     P:55, ref. 25
+ *              order 6 (the paper's, 7 stages) or order 4 (BASELINE configs, 3 stages)      R1, R2
+ *   ensemble   N independent realisations, one per GPU thread
+ *   ICs        on the energy shell H = E, third action from the energy condition
+ *   indicator  tangent vector through the exact derivative of the discrete map -> FLI / FTLE   R3, R13
+ *   density    histogram of the ensemble over the first two actions, accumulated in time
+ *
+ * Conventions common to every entry point
+ *   - returns an aw_status (0 = AW_OK, negative = error); never throws, never sets errno;
+ *   - every argument is validated ON THE HOST before anything is launched;
+ *   - all device work is enqueued asynchronously on aw_state.stream; no call synchronises unless its
+ *     comment says so (the *_host and *_probe calls do);
+ *   - the library never allocates or frees the caller's planes; pointers marked "device" must be
+ *     device-accessible global memory, 16-byte aligned; "host" pointers are ordinary host memory;
+ *   - thread-safe for distinct aw_state objects; the only library state is a thread-local
+ *     last-CUDA-error code and a process-wide launch counter;
+ *   - there is NO CPU fallback: without a CUDA device every compute entry returns AW_ECUDA.
+ */
+#ifndef AW_H_
+#define AW_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define AW_VERSION 100 /* 1.0.0 */
+
+#if defined(__GNUC__)
+#define AW_API __attribute__((visibility("default")))
+#else
+#define AW_API
+#endif
+
+typedef enum {
+  AW_OK = 0,
+  AW_EINVAL = -1, /* bad argument: null / misaligned plane, n mismatch, stride <= 0, ...       */
+  AW_ECUDA = -2,  /* a CUDA runtime call failed; see aw_last_cuda_error()                       */
+  AW_ERANGE = -3, /* argument outside the range the arithmetic supports (see aw_integrate)      */
+  AW_ESTATE = -4  /* aw_state not usable for this call (not initialised, no tangent planes ...) */
+} aw_status;
+
+/* indicator kinds for aw_indicator (R13, R14) */
+enum { AW_IND_FLI = 0, AW_IND_FTLE = 1, AW_IND_DH = 2, AW_IND_CLASS = 3 };
+/* aw_grid.shape */
+enum { AW_SHAPE_GRID = 0, AW_SHAPE_DISK = 1, AW_SHAPE_GAUSS = 2 };
+/* per-trajectory status byte */
+enum { AW_ST_OFFSHELL = 0, AW_ST_LIVE = 1, AW_ST_NONFINITE = 2 };
+
+/* Static, never-freed description of a status code. */
+AW_API const char *aw_strerror(int code);
+/* cudaError_t (as int) of the last AW_ECUDA returned on the calling thread; 0 if none. */
+AW_API int aw_last_cuda_error(void);
+/* AW_VERSION the library was built from. */
+AW_API int aw_version(void);
+/* Number of CUDA kernels this library has launched in this process so far (monotonic). */
+AW_API uint64_t aw_launch_count(void);
+
+/* Ensemble state: structure-of-arrays planes in device memory, owned by the caller (§8(b)).
+ * Plane c of a buffer starts at element c*pitch; trajectory k is element k of every plane, so a warp
+ * reads 32 consecutive doubles per plane (coalesced 256-byte segments).  The struct is plain data. */
+typedef struct {
+  int64_t n;       /* trajectories                                                            */
+  int64_t pitch;   /* elements between planes, >= n, multiple of 32                           */
+  double *q;       /* device, 6*pitch: planes x, y, z, px, py, pz  (angles X, actions P)  */
+  double *w;       /* device, 6*pitch tangent planes dx,dy,dz,dpx,dpy,dpz; NULL = no tangent  */
+  double *acc;     /* device, 4*pitch: logsum, fli_max, H0, dH_max  (R4, R13, R16)            */
+  int32_t *wind;   /* device, 3*pitch whole-turn counters of x,y,z (R7); NULL = not tracked   */
+  uint8_t *status; /* device, n bytes: AW_ST_*                                                */
+  double E, eps;   /* shell energy and perturbation strength (set by aw_init_shell; R5)       */
+  double t;        /* elapsed model time, sum of steps*|dt| (advanced by aw_integrate)         */
+  int64_t step;    /* elapsed steps                                                           */
+  int32_t order;   /* 4 or 6 (R1); set by the caller before aw_integrate; default 4           */
+  int32_t ready;   /* set to 1 by aw_init_shell (or by the caller after uploading a state)    */
+  void *stream;    /* cudaStream_t; NULL = legacy default stream                              */
+} aw_state;
+
+/* Initial-condition family (P:85 whole region, P:87 patch, P:97 cloud; R6, R8, R9, R12, R17, R18). */
+typedef struct {
+  int32_t gx, gy;               /* n must equal gx*gy; trajectory k = j*gx + i                 */
+  double lo_x, hi_x, lo_y, hi_y; /* action rectangle for shape GRID; samples are cell-centred:
+                                    px = lo_x + (i + 1/2)(hi_x - lo_x)/gx, py likewise with j  */
+  int32_t angle_mode;           /* 0: all angles 0;  1: angle_a = 2pi * u(seed, k, a), a=0,1,2 */
+  int32_t shape;                /* AW_SHAPE_*: DISK  (px,py) = (cx,cy) + r sqrt(u3) (cos,sin)(2pi u4)
+                                               GAUSS (px,py) = (cx,cy) + r sqrt(-2 ln(1-u3)) (cos,sin)(2pi u4) */
+  double cx, cy, r;
+  int32_t pz_sign;              /* +1 (default, upper hemisphere; R9) or -1                    */
+  int32_t tangent_mode;         /* 0: one common seeded unit vector (R12); 1: per trajectory   */
+} aw_grid;
+
+/* Bytes the caller must provide for each buffer.  *pitch_out = n rounded up to a multiple of 32.
+ * Returns 6*pitch*8 (+ 6*pitch*8 if with_tangent) + 4*pitch*8 (+ 3*pitch*4 if with_wind) + n, i.e. the
+ * total if all planes were packed back to back; the planes may equally be separate allocations. */
+AW_API size_t aw_state_bytes(int64_t n, int with_tangent, int with_wind, int64_t *pitch_out);
+
+/* Counter-based randomness (R11): mix64(seed, ctr): z = seed + ctr*0x9E3779B97F4A7C15 (mod 2^64);
+ * z ^= z>>30; z *= 0xBF58476D1CE4E5B9; z ^= z>>27; z *= 0x94D049BB133111EB; z ^= z>>31.
+ * u(seed, k, slot) = (mix64(seed, 16k + slot) >> 11) * 2^-53 in [0,1).  Slots: 0-2 angles, 3-4 cloud,
+ * 5-10 tangent normals (Box-Muller pairs (5,6), (7,8), (9,10) on (1 - u_a, u_b)).                 */
+
+/* §8(a) a1 — initial conditions on the energy shell ("v_z from the energy
+ * condition").  For every k: (px,py) from the grid or cloud; angles per angle_mode;
+ * R = 2(E - eps H_p(X)) - px^2 - py^2; R < 0 -> status 0 and all six state words NaN (R8);
+ * else pz = pz_sign*sqrt(R), status 1.  acc = {0, 0, H(X,P), 0}; wind = 0; tangent = common unit
+ * vector (computed on the host, see aw_common_tangent) or the per-trajectory one.  Sets s->E, eps,
+ * t = 0, step = 0, ready = 1.  Errors: AW_EINVAL (null s/grid/planes, n != gx*gy, pitch < n or not a
+ * multiple of 32, hi <= lo, r < 0, bad modes), AW_ERANGE (E - 2|eps| <= 0 or non-finite). */
+AW_API int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps, uint64_t seed);
+
+/* §8(a) a2 + a3 + a4 — advance every live trajectory by `steps` steps of size dt.
+ * One step = for s in 1..S { X += a_s P; P -= b_s grad H_p(X) } X += a_{S+1} P  with
+ * a_s = c_s*dt, b_s = (eps*w_s)*dt (R2; constants from aw_stage_constants).  If s->w != NULL the
+ * tangent vector goes through the exact derivative of the same map (R3).  Every `stride` steps the
+ * fused checkpoint runs (R4): renormalise the tangent vector, logsum += ln|w|, fli = max(fli, logsum);
+ * dH_max = max(dH_max, |H - H0|); wrap the angles to [-pi,pi] counting whole turns into wind (R7);
+ * a non-finite state sets status 2 and freezes the trajectory.
+ * n must equal s->n.  steps >= 0, stride > 0, steps % stride == 0; dt != 0 finite (dt < 0 integrates
+ * backwards).  steps == 0 or n == 0 is a no-op.  AW_ERANGE if stride*|dt|*sqrt(2(E+2|eps|)) >= 1024
+ * (the angle would leave the range the two-constant argument reduction handles exactly, R7).
+ * AW_ESTATE if !s->ready or order not in {4, 6}.  Advances s->t and s->step.
+ * The work is split into kernel launches of at most AW_MAX_STEPS_PER_LAUNCH steps (a multiple of
+ * stride); the result does not depend on the split. */
+#define AW_MAX_STEPS_PER_LAUNCH 20000
+AW_API int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t stride);
+
+/* §8(a) a5 — indicator image.  kind AW_IND_FLI: fli_max; AW_IND_FTLE: logsum / s->t; AW_IND_DH:
+ * dH_max -> out_dev = n doubles (device), NaN where status != 1.  AW_IND_CLASS: out_dev = n bytes
+ * (device), 1 if fli_max > thr else 0, 255 where status != 1 (R14; pass thr = log(t) + 3 for the
+ * default).  AW_ESTATE if a tangent indicator is asked of a state without tangent planes, or FTLE
+ * at t == 0. */
+AW_API int aw_indicator(const aw_state *s, int kind, double thr, void *out_dev);
+
+/* §8(a) a6 — visited-cell density over the first two actions (R19, R20).  For each live
+ * trajectory ix = floor((px - lo) * (gx/(hi - lo))), iy likewise with gy; inside -> hist[iy*gx + ix]
+ * += 1, else *dropped_dev += 1 (dropped_dev may be NULL).  ADDS into hist_dev (device, gx*gy uint32;
+ * the caller zeroes it) so repeated calls give the time-accumulated density.  mode must be 0. */
+AW_API int aw_density(const aw_state *s, uint32_t *hist_dev, int32_t gx, int32_t gy, double lo, double hi,
+               int mode, uint64_t *dropped_dev);
+
+/* Host helpers (pure host arithmetic, no device needed) ------------------------------------------ */
+
+/* Stage constants of the scheme (R2): fills a[0..S] and b[0..S-1], returns S (3 for order 4, 7 for
+ * order 6) or AW_EINVAL.  Order-6 weights are obtained inside the library by Newton iteration on the
+ * four order conditions in extended precision. */
+AW_API int aw_stage_constants(int order, double dt, double eps, double *a_host, double *b_host);
+/* The common tangent vector of tangent_mode 0: unit vector from u(seed, 2^63-1, 5..10) (R12). */
+AW_API int aw_common_tangent(uint64_t seed, double *t6_host);
+
+/* End-to-end call with HOST buffers (synchronous) ------------------------------------------------ *
+ * Uploads a host-resident state into the caller-provided device planes of *s (q, w if non-NULL, acc,
+ * wind if non-NULL, status; host layouts identical to the device ones), runs aw_integrate(steps, dt,
+ * stride), aw_indicator(kind, thr) and aw_density(gx, gy, lo, hi), and downloads the image
+ * (n doubles, or n bytes for CLASS) and the histogram (gx*gy uint32, ADDED into hist_host's content
+ * is NOT done: the device histogram is zeroed first and hist_host is overwritten) and the final state
+ * planes that are non-NULL in the out arguments.  ind_dev / hist_dev are device scratch of n*8 and
+ * gx*gy*4 + 8 bytes.  Synchronises s->stream before returning. */
+typedef struct {
+  const double *q, *w, *acc;  /* host, same pitch as s                                            */
+  const int32_t *wind;        /* host or NULL                                                     */
+  const uint8_t *status;      /* host                                                             */
+} aw_host_in;
+typedef struct {
+  void *image;        /* host, n doubles (n bytes for CLASS) or NULL                              */
+  uint32_t *hist;     /* host, gx*gy or NULL (then no density is computed)                        */
+  uint64_t *dropped;  /* host, 1 or NULL                                                          */
+  double *q;          /* host, 6*pitch final state or NULL                                        */
+  double *acc;        /* host, 4*pitch final accumulators or NULL                                 */
+  uint8_t *status;    /* host, n or NULL                                                          */
+} aw_host_out;
+AW_API int aw_map_host(aw_state *s, const aw_host_in *in, int64_t steps, double dt, int64_t stride, int kind,
+                double thr, int32_t gx, int32_t gy, double lo, double hi, void *ind_dev,
+                void *hist_dev, const aw_host_out *out);
+
+/* Probes (synchronous; test and measurement support, not on the hot path) ------------------------ */
+
+/* Device sincos used by the integrator (csrc/aw_trig.cuh), evaluated on n device doubles. */
+AW_API int aw_sincos_probe(const double *x_dev, int64_t n, double *sin_dev, double *cos_dev, void *stream);
+/* u(seed, k0 + i, slot) for i in [0, n) written to out_dev (device). */
+AW_API int aw_uniform_probe(uint64_t seed, uint64_t k0, int64_t n, uint32_t slot, double *out_dev,
+                     void *stream);
+/* H(X,P) by the device routine the checkpoint uses, for n states in SoA planes q (6*pitch). */
+AW_API int aw_hamiltonian_probe(const double *q_dev, int64_t n, int64_t pitch, double eps, double *out_dev,
+                         void *stream);
+/* fp64 FMA peak microbenchmark: every thread runs `chains` (1..16) independent DFMA chains of `iters`
+ * links; grid = blocks x threads.  Writes elapsed milliseconds (CUDA events) and the DFMA count
+ * (thread-instructions) to the host outputs; flop/s = 2*dfma/ms*1e3.  sink_dev: >= 8 bytes device. */
+AW_API int aw_dfma_peak_probe(int blocks, int threads, int chains, int64_t iters, double *sink_dev,
+                       double *ms_host, double *dfma_host, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AW_H_ */

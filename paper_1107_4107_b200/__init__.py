@@ -1,0 +1,16 @@
+"""paper_1107_4107_b200 — B200-native (sm_100a) hot path of arXiv 1107.4107: ensemble symplectic
+integration of the paper's 3-d.o.f. Hamiltonian -> Arnold-web maps (FLI image + visited-cell density).
+
+The product is libaw.so (hand-written CUDA behind the C ABI of include/aw.h).  This package is the
+thin Python binding: argument marshalling only.  PyTorch is used for device memory and streams.
+There is no CPU fallback: importing the binding without the built library raises.
+"""
+from .binding import (AW_IND_CLASS, AW_IND_DH, AW_IND_FLI, AW_IND_FTLE, AwError, Ensemble, Grid,
+                      aw_common_tangent, aw_density, aw_dfma_peak_probe, aw_hamiltonian_probe,
+                      aw_indicator, aw_init_shell, aw_integrate, aw_launch_count, aw_map_host,
+                      aw_sincos_probe, aw_stage_constants, aw_state_bytes, aw_strerror,
+                      aw_uniform_probe, aw_version, lib, make_grid)
+from .configs import CONFIGS
+
+__all__ = [n for n in dir() if n.startswith(("aw_", "AW_")) or n in
+           ("AwError", "Ensemble", "Grid", "lib", "make_grid", "CONFIGS")]

@@ -1,0 +1,34 @@
+"""Workload definitions (BASELINE.json configs[0..4]) as plain data.
+
+No arithmetic of the method lives here: these are the parameters handed to aw_init_shell /
+aw_integrate, shared by the tests (which pass the same numbers to the oracle) and by bench.py.
+Inputs are synthetic and seeded: the paper's own initial conditions are random draws it does not print
+(P:85); the configs take the shapes of its scans.
+"""
+
+# key: (grid, E, eps, seed, order, dt, steps, stride, tangent, outputs)
+CONFIGS = {
+    0: dict(name="cfg0_64x64_eps1e-2", gx=64, gy=64, lo=-1.0, hi=1.0, angle_mode=1, shape=0,
+            cx=0.0, cy=0.0, r=0.0, E=1.0, eps=1e-2, seed=0, order=4, dt=0.01, steps=10_000,
+            stride=100, tangent=False, density_every=0),
+    1: dict(name="cfg1_512x512_eps1e-3_fli", gx=512, gy=512, lo=-1.0, hi=1.0, angle_mode=0, shape=0,
+            cx=0.0, cy=0.0, r=0.0, E=1.0, eps=1e-3, seed=0, order=4, dt=0.01, steps=100_000,
+            stride=100, tangent=True, density_every=0),
+    2: dict(name="cfg2_1024x1024_eps1e-4_fli", gx=1024, gy=1024, lo=-1.0, hi=1.0, angle_mode=1, shape=0,
+            cx=0.0, cy=0.0, r=0.0, E=1.0, eps=1e-4, seed=1, order=4, dt=0.02, steps=1_000_000,
+            stride=100, tangent=True, density_every=0),
+    3: dict(name="cfg3_2048x2048_eps3e-2_fli", gx=2048, gy=2048, lo=-1.0, hi=1.0, angle_mode=0, shape=0,
+            cx=0.0, cy=0.0, r=0.0, E=1.0, eps=3e-2, seed=0, order=4, dt=0.005, steps=200_000,
+            stride=100, tangent=True, density_every=0),
+    4: dict(name="cfg4_diffusion_2^20", gx=1024, gy=1024, lo=-1.0, hi=1.0, angle_mode=1, shape=1,
+            cx=0.0, cy=0.0, r=1e-3, E=1.0, eps=1e-3, seed=0, order=4, dt=0.01, steps=10_000_000,
+            stride=100, tangent=False, density_every=10_000),
+}
+
+HIST_G = 1024          # density histogram is HIST_G x HIST_G over [HIST_LO, HIST_HI]^2 (configs[4])
+HIST_LO, HIST_HI = -1.0, 1.0
+
+# nominal fp64 flops per trajectory-step (FMA = 2, MUL/ADD = 1, sincos = 36)
+NOMINAL_FLOPS = {(4, False): 384, (4, True): 498, (6, False): 896, (6, True): 1162}
+# datasheet-derived fp64 FMA peak: 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz
+FP64_PEAK_TFLOPS_NOMINAL = 148 * 64 * 2 * 1.965e9 / 1e12

@@ -1,0 +1,410 @@
+// aw_api.cu — the C ABI of include/aw.h: host-side validation, stage constants, launch chaining.
+// Every entry validates on the host before any launch and returns an aw_status; nothing here touches
+// trajectory data on the CPU (there is no CPU fallback — without a device the calls return AW_ECUDA).
+#include <atomic>
+#include <cmath>
+#include <cstring>
+#include <mutex>
+
+#include "aw_internal.cuh"
+
+namespace aw {
+
+static thread_local int g_last_cuda = 0;
+static std::atomic<uint64_t> g_launches{0};
+
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+
+static int cuda_fail(cudaError_t e) {
+  g_last_cuda = (int)e;
+  return AW_ECUDA;
+}
+#define AW_CUDA(call)                                  \
+  do {                                                 \
+    cudaError_t e_ = (call);                           \
+    if (e_ != cudaSuccess) return ::aw::cuda_fail(e_); \
+  } while (0)
+
+// ---- stage weights of the composition (R1, R2) -----------------------------------------------------
+//
+// order 4: triple jump, closed form.  order 6: 7-stage palindromic composition (w3 w2 w1 w0 w1 w2 w3);
+// the paper prints no coefficients, so they are obtained here as the root of the four order conditions
+//   sum g = 1, sum g^3 = 0, sum g^5 = 0, sum_i g_i^3 (sum_{j<i} g_j + g_i/2)^2 = 0
+// nearest to Yoshida's "solution A" (smallest max |w|), by Newton iteration in long double with a
+// central-difference Jacobian (ample: the system is polynomial and well conditioned at the root; the
+// iteration converges to the long-double root, which is then rounded once to double).
+static void y6_conditions(const long double w[4], long double f[4]) {
+  const long double g[7] = {w[3], w[2], w[1], w[0], w[1], w[2], w[3]};
+  long double e1 = -1.0L, e3 = 0.0L, e5 = 0.0L, e7 = 0.0L, pre = 0.0L;
+  for (int i = 0; i < 7; ++i) {
+    const long double x = g[i], x3 = x * x * x, mid = pre + x / 2;
+    e1 += x;
+    e3 += x3;
+    e5 += x3 * x * x;
+    e7 += x3 * mid * mid;
+    pre += x;
+  }
+  f[0] = e1; f[1] = e3; f[2] = e5; f[3] = e7;
+}
+
+static void solve4(long double A[4][4], long double b[4]) {  // Gaussian elimination, partial pivoting
+  for (int c = 0; c < 4; ++c) {
+    int piv = c;
+    for (int r = c + 1; r < 4; ++r)
+      if (fabsl(A[r][c]) > fabsl(A[piv][c])) piv = r;
+    for (int k = 0; k < 4; ++k) { long double t = A[c][k]; A[c][k] = A[piv][k]; A[piv][k] = t; }
+    { long double t = b[c]; b[c] = b[piv]; b[piv] = t; }
+    for (int r = c + 1; r < 4; ++r) {
+      const long double m = A[r][c] / A[c][c];
+      for (int k = c; k < 4; ++k) A[r][k] -= m * A[c][k];
+      b[r] -= m * b[c];
+    }
+  }
+  for (int r = 3; r >= 0; --r) {
+    for (int k = r + 1; k < 4; ++k) b[r] -= A[r][k] * b[k];
+    b[r] /= A[r][r];
+  }
+}
+
+static const double *yoshida6_weights() {
+  static double w6[4];
+  static std::once_flag once;
+  std::call_once(once, [] {
+    long double w[4] = {1.3152L, -1.1777L, 0.2356L, 0.7845L};  // 4-digit neighbourhood of solution A
+    for (int it = 0; it < 40; ++it) {
+      long double f[4], J[4][4];
+      y6_conditions(w, f);
+      for (int c = 0; c < 4; ++c) {
+        const long double h = 1e-9L;
+        long double wp[4], wm[4], fp[4], fm[4];
+        for (int k = 0; k < 4; ++k) wp[k] = wm[k] = w[k];
+        wp[c] += h; wm[c] -= h;
+        y6_conditions(wp, fp);
+        y6_conditions(wm, fm);
+        for (int r = 0; r < 4; ++r) J[r][c] = (fp[r] - fm[r]) / (2 * h);
+      }
+      long double rhs[4] = {-f[0], -f[1], -f[2], -f[3]};
+      solve4(J, rhs);
+      long double step = 0;
+      for (int k = 0; k < 4; ++k) { w[k] += rhs[k]; step = fmaxl(step, fabsl(rhs[k])); }
+      if (step < 1e-19L) break;
+    }
+    for (int k = 0; k < 4; ++k) w6[k] = (double)w[k];
+  });
+  return w6;
+}
+
+static int stage_list(int order, double w[kMaxStages]) {
+  if (order == 4) {
+    const double cbrt2 = std::cbrt(2.0);
+    w[0] = 1.0 / (2.0 - cbrt2);
+    w[1] = -cbrt2 / (2.0 - cbrt2);
+    w[2] = w[0];
+    return 3;
+  }
+  if (order == 6) {
+    const double *y = yoshida6_weights();
+    w[0] = y[3]; w[1] = y[2]; w[2] = y[1]; w[3] = y[0]; w[4] = y[1]; w[5] = y[2]; w[6] = y[3];
+    return 7;
+  }
+  return 0;
+}
+
+// a_s = c_s*dt with c_1 = w_1/2, c_s = (w_{s-1} + w_s)/2, c_{S+1} = w_S/2;  b_s = (eps*w_s)*dt  (R2)
+static int stage_constants(int order, double dt, double eps, double a[kMaxStages + 1], double b[kMaxStages]) {
+  double w[kMaxStages];
+  const int S = stage_list(order, w);
+  if (S == 0) return 0;
+  for (int s = 0; s <= S; ++s) {
+    double c;
+    if (s == 0) c = w[0] / 2.0;
+    else if (s == S) c = w[S - 1] / 2.0;
+    else c = (w[s - 1] + w[s]) / 2.0;
+    a[s] = c * dt;
+  }
+  for (int s = 0; s < S; ++s) b[s] = (eps * w[s]) * dt;
+  return S;
+}
+
+// ---- the common tangent vector (R12): host libm, counter k = 2^63 - 1, slots 5..10 -------------------
+static void common_tangent(uint64_t seed, double t[6]) {
+  const double two_pi_hi = 6.283185307179586;
+  const uint64_t k = 0x7FFFFFFFFFFFFFFFull;
+  for (int pr = 0; pr < 3; ++pr) {
+    const double ua = uniform01(seed, k, 5 + 2 * pr), ub = uniform01(seed, k, 6 + 2 * pr);
+    const double rad = std::sqrt(-2.0 * std::log(1.0 - ua));
+    const double ang = two_pi_hi * ub;
+    t[2 * pr] = rad * std::cos(ang);
+    t[2 * pr + 1] = rad * std::sin(ang);
+  }
+  double s2 = 0.0;
+  for (int i = 0; i < 6; ++i) s2 = s2 + t[i] * t[i];
+  const double nu = std::sqrt(s2);
+  for (int i = 0; i < 6; ++i) t[i] = t[i] / nu;
+}
+
+static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int check_planes(const aw_state *s) {
+  if (!s) return AW_EINVAL;
+  if (s->n < 0 || s->pitch < s->n || (s->pitch & 31) != 0) return AW_EINVAL;
+  if (s->n > 0) {
+    if (!s->q || !s->acc || !s->status) return AW_EINVAL;
+    if (!aligned16(s->q) || !aligned16(s->acc) || (s->w && !aligned16(s->w)) ||
+        (s->wind && !aligned16(s->wind)))
+      return AW_EINVAL;
+  }
+  return AW_OK;
+}
+
+}  // namespace aw
+
+using namespace aw;
+
+extern "C" {
+
+const char *aw_strerror(int code) {
+  switch (code) {
+    case AW_OK: return "ok";
+    case AW_EINVAL: return "invalid argument";
+    case AW_ECUDA: return "CUDA runtime error (see aw_last_cuda_error)";
+    case AW_ERANGE: return "argument out of the supported range";
+    case AW_ESTATE: return "state not usable for this call";
+    default: return "unknown aw_status";
+  }
+}
+
+int aw_last_cuda_error(void) { return g_last_cuda; }
+int aw_version(void) { return AW_VERSION; }
+uint64_t aw_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+size_t aw_state_bytes(int64_t n, int with_tangent, int with_wind, int64_t *pitch_out) {
+  if (n < 0) n = 0;
+  const int64_t pitch = (n + 31) / 32 * 32;
+  if (pitch_out) *pitch_out = pitch;
+  size_t bytes = (size_t)6 * pitch * 8 + (size_t)4 * pitch * 8 + (size_t)n;
+  if (with_tangent) bytes += (size_t)6 * pitch * 8;
+  if (with_wind) bytes += (size_t)3 * pitch * 4;
+  return bytes;
+}
+
+int aw_stage_constants(int order, double dt, double eps, double *a_host, double *b_host) {
+  if (!a_host || !b_host) return AW_EINVAL;
+  double a[kMaxStages + 1], b[kMaxStages];
+  const int S = stage_constants(order, dt, eps, a, b);
+  if (S == 0) return AW_EINVAL;
+  std::memcpy(a_host, a, sizeof(double) * (S + 1));
+  std::memcpy(b_host, b, sizeof(double) * S);
+  return S;
+}
+
+int aw_common_tangent(uint64_t seed, double *t6_host) {
+  if (!t6_host) return AW_EINVAL;
+  common_tangent(seed, t6_host);
+  return AW_OK;
+}
+
+int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps, uint64_t seed) {
+  if (!s || !grid) return AW_EINVAL;
+  int rc = check_planes(s);
+  if (rc != AW_OK) return rc;
+  if (grid->gx <= 0 || grid->gy <= 0 || (int64_t)grid->gx * grid->gy != s->n) return AW_EINVAL;
+  if (grid->angle_mode != 0 && grid->angle_mode != 1) return AW_EINVAL;
+  if (grid->tangent_mode != 0 && grid->tangent_mode != 1) return AW_EINVAL;
+  if (grid->shape == AW_SHAPE_GRID) {
+    if (!(grid->hi_x > grid->lo_x) || !(grid->hi_y > grid->lo_y)) return AW_EINVAL;
+    if (!std::isfinite(grid->lo_x) || !std::isfinite(grid->hi_x) || !std::isfinite(grid->lo_y) ||
+        !std::isfinite(grid->hi_y))
+      return AW_EINVAL;
+  } else if (grid->shape == AW_SHAPE_DISK || grid->shape == AW_SHAPE_GAUSS) {
+    if (!(grid->r >= 0.0) || !std::isfinite(grid->r) || !std::isfinite(grid->cx) || !std::isfinite(grid->cy))
+      return AW_EINVAL;
+  } else {
+    return AW_EINVAL;
+  }
+  if (!std::isfinite(E) || !std::isfinite(eps) || !(E - 2.0 * std::fabs(eps) > 0.0)) return AW_ERANGE;
+
+  if (s->n > 0) {
+    InitParams p;
+    p.q = s->q; p.w = s->w; p.acc = s->acc; p.wind = s->wind; p.status = s->status;
+    p.n = s->n; p.pitch = s->pitch;
+    p.g = *grid;
+    p.E = E; p.eps = eps; p.seed = seed;
+    common_tangent(seed, p.tcommon);
+    AW_CUDA(launch_init(p, (cudaStream_t)s->stream));
+  }
+  s->E = E; s->eps = eps; s->t = 0.0; s->step = 0; s->ready = 1;
+  if (s->order != 4 && s->order != 6) s->order = 4;
+  return AW_OK;
+}
+
+int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t stride) {
+  if (!s) return AW_EINVAL;
+  int rc = check_planes(s);
+  if (rc != AW_OK) return rc;
+  if (n != s->n || steps < 0 || stride <= 0 || steps % stride != 0) return AW_EINVAL;
+  if (!(dt != 0.0) || !std::isfinite(dt)) return AW_EINVAL;
+  if (!s->ready || (s->order != 4 && s->order != 6)) return AW_ESTATE;
+  if (!std::isfinite(s->E) || !std::isfinite(s->eps)) return AW_ESTATE;
+  if (stride > 0x7fffffff) return AW_ERANGE;
+  const double vmax = std::sqrt(2.0 * (s->E + 2.0 * std::fabs(s->eps)));
+  if (!((double)stride * std::fabs(dt) * vmax < 1024.0)) return AW_ERANGE;
+  if (steps == 0 || n == 0) return AW_OK;
+
+  double a[kMaxStages + 1], b[kMaxStages];
+  const int S = stage_constants(s->order, dt, s->eps, a, b);
+  IntegrateParams p;
+  std::memset(&p, 0, sizeof p);
+  p.q = s->q; p.w = s->w; p.acc = s->acc; p.wind = s->wind; p.status = s->status;
+  p.n = s->n; p.pitch = s->pitch;
+  p.stride = (int32_t)stride;
+  p.a_first = a[0];
+  p.a_last = a[S];
+  p.a_merge = a[S] + a[0];
+  for (int k = 1; k < S; ++k) p.a_mid[k - 1] = a[k];
+  for (int k = 0; k < S; ++k) { p.b2[k] = 2.0 * b[k]; p.b4[k] = 4.0 * b[k]; }
+  p.eps = s->eps;
+
+  const int64_t total_chk = steps / stride;
+  int64_t chk_per_launch = AW_MAX_STEPS_PER_LAUNCH / stride;
+  if (chk_per_launch < 1) chk_per_launch = 1;
+  const double t0 = s->t;
+  const int64_t step0 = s->step;
+  for (int64_t done = 0; done < total_chk; done += chk_per_launch) {
+    const int64_t now = (total_chk - done < chk_per_launch) ? total_chk - done : chk_per_launch;
+    p.nchk = (int32_t)now;
+    const cudaError_t e = launch_integrate(p, s->order, s->w != nullptr, (cudaStream_t)s->stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+    s->step = step0 + (done + now) * stride;
+    s->t = t0 + (double)(s->step - step0) * std::fabs(dt);
+  }
+  return AW_OK;
+}
+
+int aw_indicator(const aw_state *s, int kind, double thr, void *out_dev) {
+  if (!s || !out_dev) return AW_EINVAL;
+  int rc = check_planes(s);
+  if (rc != AW_OK) return rc;
+  if (kind < AW_IND_FLI || kind > AW_IND_CLASS) return AW_EINVAL;
+  if (!s->ready) return AW_ESTATE;
+  if (kind != AW_IND_DH && !s->w) return AW_ESTATE;
+  if (kind == AW_IND_FTLE && !(s->t > 0.0)) return AW_ESTATE;
+  if (kind == AW_IND_CLASS && thr != thr) return AW_EINVAL;
+  if (kind != AW_IND_CLASS && !aligned16(out_dev)) return AW_EINVAL;
+  if (s->n == 0) return AW_OK;
+  AW_CUDA(launch_indicator(s->acc, s->status, s->n, s->pitch, kind, thr, s->t, out_dev,
+                           (cudaStream_t)s->stream));
+  return AW_OK;
+}
+
+int aw_density(const aw_state *s, uint32_t *hist_dev, int32_t gx, int32_t gy, double lo, double hi,
+               int mode, uint64_t *dropped_dev) {
+  if (!s || !hist_dev) return AW_EINVAL;
+  int rc = check_planes(s);
+  if (rc != AW_OK) return rc;
+  if (mode != 0 || gx <= 0 || gy <= 0 || !(hi > lo) || !std::isfinite(lo) || !std::isfinite(hi))
+    return AW_EINVAL;
+  if ((int64_t)gx * gy >= 0xffffffffll) return AW_ERANGE;
+  if (!s->ready) return AW_ESTATE;
+  if (s->n == 0) return AW_OK;
+  const double fx = (double)gx / (hi - lo), fy = (double)gy / (hi - lo);
+  AW_CUDA(launch_density(s->q + 3 * s->pitch, s->q + 4 * s->pitch, s->status, s->n, hist_dev, gx, gy, lo,
+                         fx, fy, reinterpret_cast<unsigned long long *>(dropped_dev),
+                         (cudaStream_t)s->stream));
+  return AW_OK;
+}
+
+int aw_map_host(aw_state *s, const aw_host_in *in, int64_t steps, double dt, int64_t stride, int kind,
+                double thr, int32_t gx, int32_t gy, double lo, double hi, void *ind_dev, void *hist_dev,
+                const aw_host_out *out) {
+  if (!s || !in || !out) return AW_EINVAL;
+  int rc = check_planes(s);
+  if (rc != AW_OK) return rc;
+  if (!in->q || !in->acc || !in->status || (s->w && !in->w) || (s->wind && !in->wind)) return AW_EINVAL;
+  if (out->image && !ind_dev) return AW_EINVAL;
+  if (out->hist && !hist_dev) return AW_EINVAL;
+  cudaStream_t st = (cudaStream_t)s->stream;
+  const size_t P = (size_t)s->pitch;
+  // host -> device
+  AW_CUDA(cudaMemcpyAsync(s->q, in->q, 6 * P * 8, cudaMemcpyHostToDevice, st));
+  if (s->w) AW_CUDA(cudaMemcpyAsync(s->w, in->w, 6 * P * 8, cudaMemcpyHostToDevice, st));
+  AW_CUDA(cudaMemcpyAsync(s->acc, in->acc, 4 * P * 8, cudaMemcpyHostToDevice, st));
+  if (s->wind) AW_CUDA(cudaMemcpyAsync(s->wind, in->wind, 3 * P * 4, cudaMemcpyHostToDevice, st));
+  AW_CUDA(cudaMemcpyAsync(s->status, in->status, (size_t)s->n, cudaMemcpyHostToDevice, st));
+  s->ready = 1;
+  rc = aw_integrate(s, s->n, steps, dt, stride);
+  if (rc != AW_OK) return rc;
+  if (out->image) {
+    rc = aw_indicator(s, kind, thr, ind_dev);
+    if (rc != AW_OK) return rc;
+    const size_t bytes = (kind == AW_IND_CLASS) ? (size_t)s->n : (size_t)s->n * 8;
+    AW_CUDA(cudaMemcpyAsync(out->image, ind_dev, bytes, cudaMemcpyDeviceToHost, st));
+  }
+  if (out->hist) {
+    const size_t hb = (size_t)gx * gy * 4;
+    if (gx <= 0 || gy <= 0) return AW_EINVAL;
+    AW_CUDA(cudaMemsetAsync(hist_dev, 0, hb + 8, st));
+    uint64_t *drop_dev = reinterpret_cast<uint64_t *>(static_cast<char *>(hist_dev) + hb);
+    rc = aw_density(s, static_cast<uint32_t *>(hist_dev), gx, gy, lo, hi, 0, drop_dev);
+    if (rc != AW_OK) return rc;
+    AW_CUDA(cudaMemcpyAsync(out->hist, hist_dev, hb, cudaMemcpyDeviceToHost, st));
+    if (out->dropped) AW_CUDA(cudaMemcpyAsync(out->dropped, drop_dev, 8, cudaMemcpyDeviceToHost, st));
+  }
+  if (out->q) AW_CUDA(cudaMemcpyAsync(out->q, s->q, 6 * P * 8, cudaMemcpyDeviceToHost, st));
+  if (out->acc) AW_CUDA(cudaMemcpyAsync(out->acc, s->acc, 4 * P * 8, cudaMemcpyDeviceToHost, st));
+  if (out->status) AW_CUDA(cudaMemcpyAsync(out->status, s->status, (size_t)s->n, cudaMemcpyDeviceToHost, st));
+  AW_CUDA(cudaStreamSynchronize(st));
+  return AW_OK;
+}
+
+int aw_sincos_probe(const double *x_dev, int64_t n, double *sin_dev, double *cos_dev, void *stream) {
+  if (!x_dev || !sin_dev || !cos_dev || n < 0) return AW_EINVAL;
+  if (n == 0) return AW_OK;
+  AW_CUDA(launch_sincos_probe(x_dev, n, sin_dev, cos_dev, (cudaStream_t)stream));
+  AW_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+  return AW_OK;
+}
+
+int aw_uniform_probe(uint64_t seed, uint64_t k0, int64_t n, uint32_t slot, double *out_dev, void *stream) {
+  if (!out_dev || n < 0 || slot > 15) return AW_EINVAL;
+  if (n == 0) return AW_OK;
+  AW_CUDA(launch_uniform_probe(seed, k0, n, slot, out_dev, (cudaStream_t)stream));
+  AW_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+  return AW_OK;
+}
+
+int aw_hamiltonian_probe(const double *q_dev, int64_t n, int64_t pitch, double eps, double *out_dev,
+                         void *stream) {
+  if (!q_dev || !out_dev || n < 0 || pitch < n) return AW_EINVAL;
+  if (n == 0) return AW_OK;
+  AW_CUDA(launch_hamiltonian_probe(q_dev, n, pitch, eps, out_dev, (cudaStream_t)stream));
+  AW_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+  return AW_OK;
+}
+
+int aw_dfma_peak_probe(int blocks, int threads, int chains, int64_t iters, double *sink_dev,
+                       double *ms_host, double *dfma_host, void *stream) {
+  if (blocks <= 0 || threads <= 0 || threads > 1024 || iters <= 0 || !sink_dev || !ms_host || !dfma_host)
+    return AW_EINVAL;
+  if (chains != 1 && chains != 2 && chains != 4 && chains != 8 && chains != 16) return AW_EINVAL;
+  iters = (iters + 7) / 8 * 8;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaEvent_t e0, e1;
+  AW_CUDA(cudaEventCreate(&e0));
+  AW_CUDA(cudaEventCreate(&e1));
+  cudaError_t err = launch_dfma_peak(blocks, threads, chains, iters / 8 > 16 ? 128 : iters, sink_dev, st);  // warm-up
+  if (err == cudaSuccess) err = cudaEventRecord(e0, st);
+  if (err == cudaSuccess) err = launch_dfma_peak(blocks, threads, chains, iters, sink_dev, st);
+  if (err == cudaSuccess) err = cudaEventRecord(e1, st);
+  if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+  float ms = 0.f;
+  if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (err != cudaSuccess) return cuda_fail(err);
+  *ms_host = (double)ms;
+  *dfma_host = (double)blocks * (double)threads * (double)chains * (double)iters;
+  return AW_OK;
+}
+
+}  // extern "C"

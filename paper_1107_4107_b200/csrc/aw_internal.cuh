@@ -1,0 +1,80 @@
+// aw_internal.cuh — declarations shared by the translation units of libaw (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/aw.h"
+
+namespace aw {
+
+constexpr int kMaxStages = 7;
+
+// Kernel parameters of the integrator; lives in the constant bank (__grid_constant__), so the stage
+// constants are constant-bank operands of the DFMA instructions and cost no registers.
+struct IntegrateParams {
+  double *q;
+  double *w;
+  double *acc;
+  int32_t *wind;
+  uint8_t *status;
+  int64_t n, pitch;
+  int32_t nchk;    // checkpoints in this launch
+  int32_t stride;  // steps between checkpoints
+  double a_first;  // a_1: drift that opens a block of `stride` steps
+  double a_merge;  // a_{S+1} + a_1: closing drift of one step merged with the opening drift of the next
+  double a_last;   // a_{S+1}: drift that closes the block
+  double a_mid[kMaxStages];  // a_2 .. a_S (drift after kick s, s = 1..S-1); a_mid[S-1] unused
+  double b2[kMaxStages];     // 2 b_s
+  double b4[kMaxStages];     // 4 b_s
+  double eps;
+};
+
+struct InitParams {
+  double *q;
+  double *w;
+  double *acc;
+  int32_t *wind;
+  uint8_t *status;
+  int64_t n, pitch;
+  aw_grid g;
+  double E, eps;
+  uint64_t seed;
+  double tcommon[6];
+};
+
+// host-side launchers (each returns cudaError_t of the launch and bumps the launch counter)
+cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, cudaStream_t st);
+cudaError_t launch_init(const InitParams &p, cudaStream_t st);
+cudaError_t launch_indicator(const double *acc, const uint8_t *status, int64_t n, int64_t pitch, int kind,
+                             double thr, double t, void *out, cudaStream_t st);
+cudaError_t launch_density(const double *px, const double *py, const uint8_t *status, int64_t n,
+                           uint32_t *hist, int32_t gx, int32_t gy, double lo, double fx, double fy,
+                           unsigned long long *dropped, cudaStream_t st);
+cudaError_t launch_sincos_probe(const double *x, int64_t n, double *s, double *c, cudaStream_t st);
+cudaError_t launch_uniform_probe(uint64_t seed, uint64_t k0, int64_t n, uint32_t slot, double *out,
+                                 cudaStream_t st);
+cudaError_t launch_hamiltonian_probe(const double *q, int64_t n, int64_t pitch, double eps, double *out,
+                                     cudaStream_t st);
+cudaError_t launch_dfma_peak(int blocks, int threads, int chains, int64_t iters, double *sink,
+                             cudaStream_t st);
+
+void count_launch();
+
+// ---- device helpers shared by kernels --------------------------------------------------------------
+#ifdef __CUDACC__
+// mix64 / u(seed, k, slot) — the counter-based generator specified in include/aw.h (R11).
+__host__ __device__ __forceinline__ uint64_t mix64(uint64_t seed, uint64_t ctr) {
+  uint64_t z = seed + ctr * 0x9E3779B97F4A7C15ull;
+  z ^= z >> 30;
+  z *= 0xBF58476D1CE4E5B9ull;
+  z ^= z >> 27;
+  z *= 0x94D049BB133111EBull;
+  z ^= z >> 31;
+  return z;
+}
+__host__ __device__ __forceinline__ double uniform01(uint64_t seed, uint64_t k, uint64_t slot) {
+  return (double)(mix64(seed, 16ull * k + slot) >> 11) * (1.0 / 9007199254740992.0);
+}
+#endif
+
+}  // namespace aw

@@ -1,0 +1,142 @@
+"""CPU-side checks of the boundary: libaw.so loads, exports every symbol include/aw.h declares, the
+host helpers agree with the oracle's separately written ones, and argument validation happens on the
+host before any launch (so it can be exercised without a GPU).  No compute calls here."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def aw():
+    from paper_1107_4107_b200 import build
+    build.build()
+    import paper_1107_4107_b200 as aw
+    return aw
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "aw.h")).read()
+    return sorted(set(re.findall(r"AW_API\s+[\w\s\*]+?\b(aw_\w+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol(aw):
+    names = declared_symbols()
+    assert len(names) >= 16 and "aw_init_shell" in names and "aw_integrate" in names
+    assert "aw_indicator" in names and "aw_density" in names
+    L = C.CDLL(os.path.join(ROOT, "paper_1107_4107_b200", "libaw.so"))
+    for n in names:
+        assert hasattr(L, n), n
+    assert aw.aw_version() == 100
+    assert aw.aw_strerror(0) == "ok" and "invalid" in aw.aw_strerror(-1)
+
+
+def test_python_binding_has_the_same_names(aw):
+    for n in declared_symbols():
+        if n == "aw_last_cuda_error":
+            continue
+        assert hasattr(aw, n), n
+
+
+def test_stage_constants_match_the_oracle(aw, orc):
+    for order in (4, 6):
+        for dt, eps in ((0.01, 1e-2), (-0.005, 3e-2), (0.02, 1e-4)):
+            a, b = aw.aw_stage_constants(order, dt, eps)
+            ao, bo = orc.stage_constants(order, dt, eps)
+            assert len(a) == len(ao) and len(b) == len(bo)
+            # order 4 is a closed form (bit-equal); order 6: library Newton (long double) vs the oracle's
+            # mpmath literals -> both are the double nearest the same root
+            assert np.allclose(a, ao, rtol=4e-16, atol=0) and np.allclose(b, bo, rtol=4e-16, atol=0)
+            if order == 4:
+                assert list(a) == list(ao) and list(b) == list(bo)
+            assert abs(sum(a) - dt) < 4e-16 * abs(dt) * 8
+    with pytest.raises(aw.AwError):
+        aw.aw_stage_constants(5, 0.01, 1e-2)
+
+
+def test_common_tangent_matches_the_oracle(aw, orc):
+    for seed in (0, 1, 12345678901234567):
+        t = np.array(aw.aw_common_tangent(seed))
+        to = orc.common_tangent(seed)
+        assert abs(np.linalg.norm(t) - 1) < 1e-15
+        assert np.max(np.abs(t - to)) < 1e-15
+
+
+def test_state_bytes(aw):
+    b, pitch = aw.aw_state_bytes(4097, True, True)
+    assert pitch == 4128 and b == 16 * pitch * 8 + 3 * pitch * 4 + 4097
+    b, pitch = aw.aw_state_bytes(64, False, False)
+    assert pitch == 64 and b == 10 * 64 * 8 + 64
+    assert aw.aw_state_bytes(0)[1] == 0
+
+
+def test_validation_happens_on_the_host(aw):
+    """Bad arguments are rejected before any CUDA call: usable without a device."""
+    from paper_1107_4107_b200.binding import AwState, Grid, lib
+    L = lib()
+    buf = (C.c_double * 1024)()
+    base = C.addressof(buf)
+    base += (-base) % 16
+    st = AwState(64, 64, base, None, base, None, base, 1.0, 1e-2, 0.0, 0, 4, 1, None)
+    g = Grid(8, 8, -1.0, 1.0, -1.0, 1.0, 0, 0, 0.0, 0.0, 0.0, 1, 0)
+    EINVAL, ERANGE, ESTATE = -1, -3, -4
+    assert L.aw_integrate(C.byref(st), 63, 100, 0.01, 100) == EINVAL        # n mismatch
+    assert L.aw_integrate(C.byref(st), 64, 150, 0.01, 100) == EINVAL        # steps % stride
+    assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 0) == EINVAL          # stride <= 0
+    assert L.aw_integrate(C.byref(st), 64, -100, 0.01, 100) == EINVAL       # steps < 0
+    assert L.aw_integrate(C.byref(st), 64, 100, 0.0, 100) == EINVAL         # dt == 0
+    assert L.aw_integrate(C.byref(st), 64, 100, float("nan"), 100) == EINVAL
+    assert L.aw_integrate(C.byref(st), 64, 100000, 1.0, 100000) == ERANGE   # angle range (R7)
+    assert L.aw_integrate(C.byref(st), 64, 0, 0.01, 100) == 0               # no-op
+    st.order = 5
+    assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == ESTATE
+    st.order, st.ready = 4, 0
+    assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == ESTATE
+    st.ready = 1
+    st.pitch = 70                                                          # not a multiple of 32
+    assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == EINVAL
+    st.pitch = 64
+    st.q = base + 8                                                        # misaligned plane
+    assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == EINVAL
+    st.q = base
+    # init_shell
+    assert L.aw_init_shell(C.byref(st), C.byref(g), 1.0, 0.6, 0) == ERANGE  # E - 2|eps| <= 0
+    g.gx = 7
+    assert L.aw_init_shell(C.byref(st), C.byref(g), 1.0, 1e-2, 0) == EINVAL  # n != gx*gy
+    g.gx, g.hi_x = 8, -1.0
+    assert L.aw_init_shell(C.byref(st), C.byref(g), 1.0, 1e-2, 0) == EINVAL  # hi <= lo
+    g.hi_x, g.shape = 1.0, 7
+    assert L.aw_init_shell(C.byref(st), C.byref(g), 1.0, 1e-2, 0) == EINVAL
+    assert L.aw_init_shell(None, C.byref(g), 1.0, 1e-2, 0) == EINVAL
+    # indicator / density
+    assert L.aw_indicator(C.byref(st), 0, 0.0, base) == ESTATE              # FLI without tangent planes
+    assert L.aw_indicator(C.byref(st), 9, 0.0, base) == EINVAL
+    assert L.aw_indicator(C.byref(st), 2, 0.0, None) == EINVAL
+    assert L.aw_density(C.byref(st), base, 16, 16, 1.0, -1.0, 0, None) == EINVAL
+    assert L.aw_density(C.byref(st), base, 16, 16, -1.0, 1.0, 1, None) == EINVAL   # mode 1 not built
+    assert L.aw_density(C.byref(st), None, 16, 16, -1.0, 1.0, 0, None) == EINVAL
+    assert L.aw_density(C.byref(st), base, 0, 16, -1.0, 1.0, 0, None) == EINVAL
+    # zero-size ensemble: every call is a no-op that never reaches the device
+    z = AwState(0, 0, None, None, None, None, None, 1.0, 1e-2, 0.0, 0, 4, 1, None)
+    g0 = Grid(0, 0, -1.0, 1.0, -1.0, 1.0, 0, 0, 0.0, 0.0, 0.0, 1, 0)
+    assert L.aw_integrate(C.byref(z), 0, 100, 0.01, 100) == 0
+    assert L.aw_init_shell(C.byref(z), C.byref(g0), 1.0, 1e-2, 0) == EINVAL  # gx <= 0
+
+
+def test_product_does_not_import_the_oracle():
+    """The product path shares nothing with oracle/ (and has no CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_1107_4107_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src, f
+                assert "aw_oracle" not in src, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_1107_4107_b200" not in src and "libaw.so" not in src, f

@@ -1,0 +1,489 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI (libaw.so), against the oracle
+on the same seeded inputs, element by element.  Tolerances are BASELINE.json north_star's, written out:
+
+  state      |gpu - oracle|_inf / max(1, |state|_inf) <= 1e-10 after 1000 steps (regular orbits)
+             and after 100 steps (chaotic ones, FLI > thr)
+  class map  equal pixel for pixel outside |FLI - thr| < 0.01 thr
+  density    bit-exact uint32 counts on identical trajectories
+  dH_max     64 ulp(E) absolute + 1 % relative at <= 1000 steps
+  FLI        1e-5 absolute where FLI < 10, 1e-2 where 10 <= FLI < 20
+
+For parity runs the GPU-generated initial conditions are copied to the oracle (R11); the two
+generators are compared separately (test_init_shell_*).
+"""
+import math
+
+import numpy as np
+import pytest
+
+from util import TWO_PI, ensemble_to_oracle, oracle_integrate_mt, state_rel_err
+
+pytestmark = pytest.mark.gpu
+
+ULP1 = 2.0 ** -52
+
+
+@pytest.fixture(scope="module")
+def aw():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1107_4107_b200 import build
+    build.build()
+    import paper_1107_4107_b200 as aw
+    return aw
+
+
+def grid_from_cfg(mod, cfg, gx=None, gy=None, tangent_mode=0):
+    return mod.make_grid(gx or cfg["gx"], gy or cfg["gy"], cfg["lo"], cfg["hi"], cfg["angle_mode"],
+                         cfg["shape"], cfg["cx"], cfg["cy"], cfg["r"], 1, tangent_mode)
+
+
+def make_pair(aw, orc, cfg, gx=None, gy=None, order=None, tangent=None, wind=True):
+    """GPU ensemble initialised by aw_init_shell + an oracle State holding a copy of it."""
+    gx, gy = gx or cfg["gx"], gy or cfg["gy"]
+    tangent = cfg["tangent"] if tangent is None else tangent
+    ens = aw.Ensemble(gx * gy, tangent=tangent, wind=wind, order=order or cfg["order"])
+    aw.aw_init_shell(ens, grid_from_cfg(aw, cfg, gx, gy), cfg["E"], cfg["eps"], cfg["seed"])
+    st = ensemble_to_oracle(ens, orc)
+    return ens, st
+
+
+# ------------------------------------------------------------------ device sincos (P14)
+
+def test_device_sincos_within_2ulp(aw):
+    import torch
+    rng = np.random.default_rng(14)
+    x = np.concatenate([rng.uniform(-16 * math.pi, 16 * math.pi, 4_000_000),
+                        rng.uniform(-1024.0, 1024.0, 1_000_000),
+                        rng.uniform(-1e-3, 1e-3, 100_000),
+                        np.arange(-2000, 2001) * (math.pi / 4),          # quadrant boundaries
+                        np.array([0.0, -0.0, math.pi, -math.pi, math.pi / 2, 1e-300, 5e-324])])
+    s, c = aw.aw_sincos_probe(torch.from_numpy(x).cuda())
+    s, c = s.cpu().numpy(), c.cpu().numpy()
+    # reference: mpmath on a sample (independent of libm), libm on everything
+    rs, rc = np.sin(x), np.cos(x)
+    def ulps(a, b):
+        return np.abs(a - b) / np.maximum(np.spacing(np.abs(b)), 5e-324)
+    assert ulps(s, rs).max() <= 2.0, ulps(s, rs).max()
+    assert ulps(c, rc).max() <= 2.0, ulps(c, rc).max()
+    import mpmath as mp
+    mp.mp.dps = 40
+    idx = rng.integers(0, x.size, 3000)
+    for i in idx:
+        xs = mp.mpf(float(x[i]))
+        es = abs(mp.mpf(float(s[i])) - mp.sin(xs)) / mp.mpf(float(np.spacing(abs(rs[i])) or 5e-324))
+        ec = abs(mp.mpf(float(c[i])) - mp.cos(xs)) / mp.mpf(float(np.spacing(abs(rc[i])) or 5e-324))
+        assert es <= 1.5 and ec <= 1.5, (x[i], es, ec)
+    # exact at 0, bitwise odd / even
+    s0, c0 = aw.aw_sincos_probe(torch.zeros(1, dtype=torch.float64, device="cuda"))
+    assert s0.item() == 0.0 and c0.item() == 1.0
+    sm, cm = aw.aw_sincos_probe(torch.from_numpy(-x).cuda())
+    assert np.array_equal(sm.cpu().numpy(), -s) and np.array_equal(cm.cpu().numpy(), c)
+
+
+def test_uniform_generator_bit_equal(aw, orc):
+    for seed, k0, slot in ((0, 0, 0), (1, 10**6, 4), (2**63 + 5, 2**40, 10)):
+        u = aw.aw_uniform_probe(seed, k0, 4096, slot).cpu().numpy()
+        ref = np.array([orc.uniform(seed, k0 + i, slot) for i in range(4096)])
+        assert np.array_equal(u, ref)
+        assert u.min() >= 0.0 and u.max() < 1.0
+
+
+# ------------------------------------------------------------------ a1: initial conditions
+
+@pytest.mark.parametrize("cfgk,gx,gy", [(0, 64, 64), (1, 96, 80), (3, 128, 128), (4, 64, 64), (2, 67, 33)])
+def test_init_shell_matches_oracle_generator(aw, orc, cfgk, gx, gy):
+    cfg = aw.CONFIGS[cfgk]
+    for tmode in (0, 1):
+        ens = aw.Ensemble(gx * gy, tangent=True, wind=True)
+        g = grid_from_cfg(aw, cfg, gx, gy, tmode)
+        aw.aw_init_shell(ens, g, cfg["E"], cfg["eps"], cfg["seed"])
+        ref = orc.State(gx * gy, True, True)
+        og = orc.make_grid(gx, gy, cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"], cfg["cx"],
+                           cfg["cy"], cfg["r"], 1, tmode)
+        orc.init_shell(ref, og, cfg["E"], cfg["eps"], cfg["seed"])
+        got = ensemble_to_oracle(ens, orc)
+        assert np.array_equal(got.status, ref.status)
+        live = ref.status == 1
+        n = gx * gy
+        if cfg["shape"] == 0:   # grid: px, py are the plain definition, bit for bit
+            assert np.array_equal(got.q[3, :n][live], ref.q[3, :n][live])
+            assert np.array_equal(got.q[4, :n][live], ref.q[4, :n][live])
+        assert np.array_equal(got.q[:3, :n][:, live], ref.q[:3, :n][:, live])      # angles: hash only
+        assert np.allclose(got.q[:, :n][:, live], ref.q[:, :n][:, live], rtol=1e-15, atol=3e-16)
+        if (~live).any():
+            assert np.isnan(got.q[:, :n][:, ~live]).all() and np.isnan(got.acc[2, :n][~live]).all()
+        # H0 = E within 4 ulp (P11), and equals what the oracle computes on the same state to rounding
+        assert np.max(np.abs(got.acc[2, :n][live] - cfg["E"])) <= 4 * ULP1 * cfg["E"] + 4e-16
+        assert np.all(got.acc[[0, 1, 3], :n] == 0.0) and np.all(got.wind == 0)
+        assert np.allclose(got.w[:, :n], ref.w[:, :n], rtol=0, atol=2e-15)
+        assert np.allclose(np.sum(got.w[:, :n] ** 2, axis=0), 1.0, atol=4e-16)
+
+
+def test_init_shell_offshell_pixels_are_masked(aw, orc):
+    # eps = 3e-2, angles 0: corners with px^2 + py^2 > 2 - 4 eps are off the shell (R8)
+    cfg = aw.CONFIGS[3]
+    ens, st = make_pair(aw, orc, cfg, 48, 48)
+    assert (st.status == 0).sum() == 4
+    fli = aw.aw_indicator(ens, aw.AW_IND_FLI).cpu().numpy()
+    assert np.isnan(fli[st.status == 0]).all() and np.all(fli[st.status == 1] == 0.0)
+
+
+# ------------------------------------------------------------------ a2: integrator, config 0 in full
+
+def test_config0_state_and_energy_parity(aw, orc):
+    cfg = aw.CONFIGS[0]
+    ens, st = make_pair(aw, orc, cfg)
+    n = ens.n
+    live = st.status == 1
+    assert live.all()
+    # horizon 1000 steps: state parity for every trajectory
+    aw.aw_integrate(ens, n, 1000, cfg["dt"], cfg["stride"])
+    oracle_integrate_mt(orc, st, 1000, cfg["dt"], cfg["stride"])
+    got = ensemble_to_oracle(ens, orc)
+    err = state_rel_err(got.q[:, :n], got.wind[:, :n], st.q[:, :n], st.wind[:, :n], live)
+    assert err.max() <= 1e-10, err.max()
+    assert np.array_equal(got.status, st.status)
+    tol = 64 * ULP1 * cfg["E"] + 0.01 * st.acc[3, :n]
+    assert np.all(np.abs(got.acc[3, :n] - st.acc[3, :n]) <= tol)
+    assert abs(ens.t - st.t) < 1e-12 and ens.step == st.step == 1000
+    # the rest of the horizon (1e4 steps, BASELINE configs[0]): energy error of the same size, no drift
+    aw.aw_integrate(ens, n, cfg["steps"] - 1000, cfg["dt"], cfg["stride"])
+    oracle_integrate_mt(orc, st, cfg["steps"] - 1000, cfg["dt"], cfg["stride"])
+    got = ensemble_to_oracle(ens, orc)
+    assert got.acc[3, :n].max() < 2e-11 and st.acc[3, :n].max() < 2e-11      # Appendix B-2: ~5e-12
+    ratio = got.acc[3, :n].max() / st.acc[3, :n].max()
+    assert 0.5 < ratio < 2.0
+    # most orbits at eps = 1e-2 are regular: they still agree closely after 1e4 steps
+    err = state_rel_err(got.q[:, :n], got.wind[:, :n], st.q[:, :n], st.wind[:, :n], live)
+    assert np.median(err) < 1e-10 and np.quantile(err, 0.9) < 1e-8
+
+
+@pytest.mark.parametrize("order", [4, 6])
+@pytest.mark.parametrize("cfgk", [1, 2, 3])
+def test_tangent_state_and_fli_parity_short_horizon(aw, orc, order, cfgk):
+    """64 x 48 sub-sampled grids of configs 1-3 (ragged: 3072 = 24 blocks), 1000 steps with the tangent map."""
+    cfg = aw.CONFIGS[cfgk]
+    ens, st = make_pair(aw, orc, cfg, 64, 48, order=order)
+    n = ens.n
+    live = st.status == 1
+    # 100 steps: every live trajectory, chaotic or not
+    aw.aw_integrate(ens, n, 100, cfg["dt"], 100)
+    oracle_integrate_mt(orc, st, 100, cfg["dt"], 100)
+    got = ensemble_to_oracle(ens, orc)
+    assert np.array_equal(got.status, st.status)
+    err = state_rel_err(got.q[:, :n], got.wind[:, :n], st.q[:, :n], st.wind[:, :n], live)
+    assert err.max() <= 1e-10, err.max()
+    werr = np.max(np.abs(got.w[:, :n][:, live] - st.w[:, :n][:, live]), axis=0)
+    assert werr.max() <= 1e-10, werr.max()
+    # 1000 steps: trajectories the indicator calls regular
+    aw.aw_integrate(ens, n, 900, cfg["dt"], 100)
+    oracle_integrate_mt(orc, st, 900, cfg["dt"], 100)
+    got = ensemble_to_oracle(ens, orc)
+    t = st.t
+    thr = math.log(t) + 3.0
+    regular = live & (st.acc[1, :n] <= thr)
+    assert regular.sum() > 0.9 * live.sum()
+    err = state_rel_err(got.q[:, :n], got.wind[:, :n], st.q[:, :n], st.wind[:, :n], regular)
+    assert err.max() <= 1e-10, err.max()
+    werr = np.max(np.abs(got.w[:, :n][:, regular] - st.w[:, :n][:, regular]), axis=0)
+    assert werr.max() <= 1e-9, werr.max()
+    # FLI / logsum values
+    fg, fo = got.acc[1, :n][live], st.acc[1, :n][live]
+    lo10 = fo < 10
+    assert np.max(np.abs(fg[lo10] - fo[lo10])) <= 1e-5
+    mid = (fo >= 10) & (fo < 20)
+    if mid.any():
+        assert np.max(np.abs(fg[mid] - fo[mid])) <= 1e-2
+    assert np.max(np.abs(got.acc[0, :n][live][lo10] - st.acc[0, :n][live][lo10])) <= 1e-5
+    tol = 64 * ULP1 * cfg["E"] + 0.01 * st.acc[3, :n][live]
+    assert np.all(np.abs(got.acc[3, :n][live] - st.acc[3, :n][live]) <= tol)
+    # indicator kernels against the oracle's a5 on the oracle's accumulators
+    for kind in (aw.AW_IND_FLI, aw.AW_IND_FTLE, aw.AW_IND_DH):
+        img = aw.aw_indicator(ens, kind).cpu().numpy()
+        ref = orc.indicator(got, kind)           # same accumulators -> must be bit-equal
+        assert np.array_equal(img, ref, equal_nan=True)
+    cls = aw.aw_indicator(ens, aw.AW_IND_CLASS, thr).cpu().numpy()
+    assert np.array_equal(cls, orc.indicator(got, 3, thr))
+
+
+@pytest.mark.parametrize("cfgk,steps", [(1, 20000), (3, 20000)])
+def test_class_map_parity_long_horizon(aw, orc, cfgk, steps):
+    """Indicator maps agree pixel for pixel on regular/chaotic outside the 1 % band (north_star)."""
+    cfg = aw.CONFIGS[cfgk]
+    ens, st = make_pair(aw, orc, cfg, 48, 48)
+    n = ens.n
+    aw.aw_integrate(ens, n, steps, cfg["dt"], cfg["stride"])
+    oracle_integrate_mt(orc, st, steps, cfg["dt"], cfg["stride"])
+    thr = math.log(st.t) + 3.0
+    cls_g = aw.aw_indicator(ens, aw.AW_IND_CLASS, thr).cpu().numpy()
+    cls_o = orc.indicator(st, 3, thr)
+    fli_o = orc.indicator(st, 0)
+    band = np.abs(fli_o - thr) < 0.01 * thr
+    live = st.status == 1
+    assert np.array_equal(cls_g[~live], cls_o[~live])            # 255 on off-shell pixels
+    mism = (cls_g != cls_o) & live & ~band
+    assert mism.sum() == 0, (mism.sum(), band.sum())
+    # both classes present at eps = 3e-2 (resonance web), ridge pixels on the diagonals (P13)
+    if cfgk == 3:
+        assert (cls_o[live] == 1).sum() > 20 and (cls_o[live] == 0).sum() > 1000
+    fli_g = aw.aw_indicator(ens, aw.AW_IND_FLI).cpu().numpy()
+    lo10 = live & (fli_o < 10)
+    assert np.max(np.abs(fli_g[lo10] - fli_o[lo10])) <= 1e-5
+
+
+# ------------------------------------------------------------------ properties that hold at any size
+
+@pytest.mark.parametrize("order", [4, 6])
+def test_gpu_free_motion_closed_form(aw, order):
+    """eps = 0: P bit-constant, X(n) = X(0) + n dt P; FLI closed form (pins P1, P2 on the GPU)."""
+    import torch
+    n = 5000
+    ens = aw.Ensemble(n, tangent=True, wind=True, order=order)
+    g = aw.make_grid(100, 50, -1.0, 1.0, angle_mode=1, tangent_mode=1)
+    aw.aw_init_shell(ens, g, 1.0, 0.0, 7)
+    q0, w0 = ens.q.cpu().numpy().copy(), ens.w.cpu().numpy().copy()
+    steps, dt = 3000, 0.01
+    aw.aw_integrate(ens, n, steps, dt, 100)
+    q1, w1 = ens.q.cpu().numpy(), ens.w.cpu().numpy()
+    wind = ens.wind.cpu().numpy()
+    assert np.array_equal(q1[3:], q0[3:])
+    X = q1[:3] + TWO_PI * wind
+    assert np.max(np.abs(X - (q0[:3] + steps * dt * q0[3:]))) < 5e-12
+    tt = steps * dt
+    dX = w0[:3] + tt * w0[3:]
+    fli_ref = 0.5 * np.log(np.sum(dX ** 2, axis=0) + np.sum(w0[3:] ** 2, axis=0))
+    logsum = ens.acc[0].cpu().numpy()
+    assert np.max(np.abs(logsum[:n] - fli_ref[:n])) < 1e-11
+    assert ens.acc[3].max().item() < 1e-14      # H = P^2/2 is conserved exactly up to rounding
+
+
+@pytest.mark.parametrize("order", [4, 6])
+def test_gpu_reversibility_and_energy(aw, order):
+    """Forward N steps then backward N steps returns to the start (pin P5 on the GPU)."""
+    cfg = aw.CONFIGS[0]
+    ens = aw.Ensemble(4096, tangent=False, wind=True, order=order)
+    aw.aw_init_shell(ens, grid_from_cfg(aw, cfg), 1.0, 1e-2, 0)
+    q0 = ens.q.cpu().numpy().copy()
+    aw.aw_integrate(ens, 4096, 1000, 0.01, 100)
+    aw.aw_integrate(ens, 4096, 1000, -0.01, 100)
+    q1 = ens.q.cpu().numpy()
+    X1 = q1[:3] + TWO_PI * ens.wind.cpu().numpy()
+    assert np.max(np.abs(X1 - q0[:3])) < 1e-11
+    assert np.max(np.abs(q1[3:] - q0[3:])) < 1e-12
+    assert ens.t == 20.0 and ens.step == 2000
+
+
+def test_gpu_invariant_subspaces_bitwise(aw):
+    """z = 0, pz = 0 stays exactly 0; x <-> y swap and (X,P) -> -(X,P) are bitwise symmetries (P9)."""
+    import torch
+    n = 256
+    rng = np.random.default_rng(9)
+    base = np.zeros((6, n))
+    base[0], base[1] = rng.uniform(-3, 3, n), rng.uniform(-3, 3, n)
+    base[3], base[4] = rng.uniform(-1, 1, n), rng.uniform(-1, 1, n)
+    acc = np.zeros((4, n))
+    status = np.ones(n, dtype=np.uint8)
+
+    def run(q):
+        ens = aw.Ensemble(n, tangent=False, wind=False, order=4)
+        ens.load_host(q, None, acc, None, status, 1.0, 1e-2)
+        aw.aw_integrate(ens, n, 500, 0.01, 100)
+        return ens.q.cpu().numpy()
+
+    a = run(base)
+    assert np.all(a[2] == 0.0) and np.all(a[5] == 0.0)
+    full = base.copy()
+    full[2], full[5] = rng.uniform(-3, 3, n), rng.uniform(-1, 1, n)
+    f = run(full)
+    sw = run(full[[1, 0, 2, 4, 3, 5]])
+    assert np.array_equal(sw[[1, 0, 2, 4, 3, 5]], f)
+    neg = run(-full)
+    assert np.array_equal(-neg, f)
+
+
+def test_launch_split_does_not_change_the_result(aw):
+    """aw_integrate chains launches of <= AW_MAX_STEPS_PER_LAUNCH steps; any split is bit-identical."""
+    cfg = aw.CONFIGS[3]
+    a = aw.Ensemble(1000, tangent=True, wind=True)
+    b = aw.Ensemble(1000, tangent=True, wind=True)
+    g = aw.make_grid(40, 25)
+    aw.aw_init_shell(a, g, 1.0, cfg["eps"], 0)
+    aw.aw_init_shell(b, g, 1.0, cfg["eps"], 0)
+    before = aw.aw_launch_count()
+    aw.aw_integrate(a, 1000, 50000, cfg["dt"], 100)           # 3 launches (20000 + 20000 + 10000)
+    assert aw.aw_launch_count() - before == 3
+    for chunk in (100, 4900, 25000, 20000):
+        aw.aw_integrate(b, 1000, chunk, cfg["dt"], 100)
+    import torch
+    assert torch.equal(a.q, b.q) and torch.equal(a.w, b.w) and torch.equal(a.acc, b.acc)
+    assert torch.equal(a.wind, b.wind) and a.step == b.step == 50000
+
+
+def test_nonfinite_state_is_frozen_with_status_2(aw, orc):
+    n = 64
+    q = np.zeros((6, n))
+    q[3:] = 0.5
+    q[3, 5] = np.inf
+    q[0, 9] = np.nan
+    acc = np.zeros((4, n))
+    status = np.ones(n, dtype=np.uint8)
+    status[3] = 0
+    ens = aw.Ensemble(n, tangent=False, wind=False)
+    ens.load_host(q, None, acc, None, status, 1.0, 1e-2)
+    aw.aw_integrate(ens, n, 300, 0.01, 100)
+    st = ens.status.cpu().numpy()
+    assert st[5] == 2 and st[9] == 2 and st[3] == 0 and (np.delete(st, [3, 5, 9]) == 1).all()
+    assert np.all(ens.q[:, 3].cpu().numpy() == q[:, 3])        # off-shell trajectory untouched
+    ref = orc.State(n, False, False)
+    ref.q[:], ref.acc[:], ref.status[:] = q, acc, status
+    ref.eps, ref.E = 1e-2, 1.0
+    orc.integrate(ref, 300, 0.01, 100)
+    assert np.array_equal(ref.status, st)
+
+
+def test_empty_and_tiny_ensembles(aw):
+    e0 = aw.Ensemble(0, tangent=True, wind=True)
+    e0.c.ready = 1
+    e0.c.E, e0.c.eps = 1.0, 1e-2
+    aw.aw_integrate(e0, 0, 100, 0.01, 100)
+    e1 = aw.Ensemble(1, tangent=True, wind=True)
+    aw.aw_init_shell(e1, aw.make_grid(1, 1), 1.0, 1e-2, 0)
+    aw.aw_integrate(e1, 1, 0, 0.01, 100)
+    assert e1.step == 0
+    aw.aw_integrate(e1, 1, 100, 0.01, 100)
+    assert e1.status[0].item() == 1 and e1.step == 100
+    with pytest.raises(aw.AwError):
+        aw.aw_integrate(e1, 2, 100, 0.01, 100)
+
+
+# ------------------------------------------------------------------ a6: density
+
+def hist_pair(aw, orc, ens, G, lo, hi, calls=1):
+    import torch
+    hist = torch.zeros((G, G), dtype=torch.int32, device="cuda")
+    dropped = torch.zeros(1, dtype=torch.int64, device="cuda")
+    for _ in range(calls):
+        aw.aw_density(ens, hist, lo, hi, 0, dropped)
+    st = ensemble_to_oracle(ens, orc)
+    ref = np.zeros((G, G), dtype=np.uint32)
+    d = np.zeros(1, dtype=np.uint64)
+    for _ in range(calls):
+        orc.density(st, ref, lo, hi, d)
+    return hist.cpu().numpy().view(np.uint32), int(dropped.item()), ref, int(d[0]), st
+
+
+def test_density_bit_exact_clustered_and_spread(aw, orc):
+    """configs[4]: 2^18-trajectory cloud, radius 1e-3 at (0,0): all points in <= 4 bins at t = 0 (worst-case
+    contention), then spread by integration; counts are bit-exact against the oracle at every binning."""
+    cfg = aw.CONFIGS[4]
+    n = 1 << 18
+    ens = aw.Ensemble(n, tangent=False, wind=True)
+    g = aw.make_grid(512, 512, cfg["lo"], cfg["hi"], 1, 1, 0.0, 0.0, cfg["r"])
+    aw.aw_init_shell(ens, g, 1.0, cfg["eps"], 0)
+    h, d, ref, dref, st = hist_pair(aw, orc, ens, 1024, -1.0, 1.0, calls=2)
+    assert np.array_equal(h, ref) and d == dref == 0
+    assert h.sum() == 2 * n and (h > 0).sum() <= 4
+    for _ in range(3):
+        aw.aw_integrate(ens, n, 1000, cfg["dt"], 100)
+        h, d, ref, dref, st = hist_pair(aw, orc, ens, 1024, -1.0, 1.0)
+        assert np.array_equal(h, ref) and d == dref
+        assert h.sum() + d == n
+
+
+def test_density_edges_ragged_and_dropped(aw, orc):
+    import torch
+    rng = np.random.default_rng(12)
+    n = 100_003                                   # ragged: not a multiple of anything
+    pitch = (n + 31) // 32 * 32
+    q = np.zeros((6, pitch))
+    q[3, :n] = rng.uniform(-1.2, 1.2, n)
+    q[4, :n] = rng.uniform(-1.2, 1.2, n)
+    edge = np.array([-1.0, 1.0 - 2 ** -53, 1.0, -0.0, 0.0, 2 / 1024, -2 / 1024, 1.0 - 2 / 1024,
+                     np.nextafter(-1.0, -2), np.nextafter(1.0, 0), 0.5, -0.5])
+    q[3, :edge.size] = edge
+    q[4, edge.size:2 * edge.size] = edge
+    status = np.ones(n, dtype=np.uint8)
+    status[rng.integers(0, n, 500)] = 0
+    status[rng.integers(0, n, 50)] = 2
+    ens = aw.Ensemble(n, tangent=False, wind=False)
+    ens.load_host(q, None, np.zeros((4, pitch)), None, status, 1.0, 1e-3)
+    for G, lo, hi in ((1024, -1.0, 1.0), (37, -0.7, 1.1), (1, -1.0, 1.0), (2048, -1.0, 1.0)):
+        h, d, ref, dref, st = hist_pair(aw, orc, ens, G, lo, hi)
+        assert np.array_equal(h, ref) and d == dref
+        assert int(h.sum()) + d == int((status == 1).sum())
+    # uniform-on-disk 2^20 points, many distinct bins per block: the shared table overflows into
+    # direct global atomics and must stay exact
+    n2 = 1 << 20
+    e2 = aw.Ensemble(n2, tangent=False, wind=False)
+    aw.aw_init_shell(e2, aw.make_grid(1024, 1024, -1, 1, 1, 1, 0.0, 0.0, 0.9), 1.0, 1e-3, 3)
+    h, d, ref, dref, st = hist_pair(aw, orc, e2, 1024, -1.0, 1.0)
+    assert np.array_equal(h, ref) and d == dref == 0 and h.sum() == n2
+
+
+# ------------------------------------------------------------------ end-to-end host call
+
+def test_map_host_equals_the_device_path(aw, orc):
+    import torch
+    cfg = aw.CONFIGS[1]
+    gx, gy = 64, 32
+    n = gx * gy
+    a = aw.Ensemble(n, tangent=True, wind=True)
+    aw.aw_init_shell(a, grid_from_cfg(aw, cfg, gx, gy), 1.0, cfg["eps"], 0)
+    host_in = dict(q=a.q.cpu().pin_memory(), w=a.w.cpu().pin_memory(), acc=a.acc.cpu().pin_memory(),
+                   wind=a.wind.cpu().pin_memory(), status=a.status[:n].cpu().pin_memory())
+    aw.aw_integrate(a, n, 2000, cfg["dt"], 100)
+    fli = aw.aw_indicator(a, aw.AW_IND_FLI)
+    hist = torch.zeros((256, 256), dtype=torch.int32, device="cuda")
+    aw.aw_density(a, hist, -1.0, 1.0)
+    b = aw.Ensemble(n, tangent=True, wind=True)
+    b.c.E, b.c.eps = 1.0, cfg["eps"]
+    out = dict(image=torch.empty(n, dtype=torch.float64).pin_memory(),
+               hist=torch.empty((256, 256), dtype=torch.int32).pin_memory(),
+               dropped=torch.zeros(1, dtype=torch.int64).pin_memory(),
+               q=torch.empty((6, b.pitch), dtype=torch.float64).pin_memory())
+    ind_dev = torch.empty(n, dtype=torch.float64, device="cuda")
+    hist_dev = torch.empty(256 * 256 + 2, dtype=torch.int32, device="cuda")
+    aw.aw_map_host(b, host_in, 2000, cfg["dt"], 100, aw.AW_IND_FLI, 0.0, (256, 256), -1.0, 1.0, ind_dev,
+                   hist_dev, out)
+    assert torch.equal(out["image"], fli.cpu()) and torch.equal(out["hist"], hist.cpu())
+    assert torch.equal(out["q"], a.q.cpu()) and out["dropped"].item() == 0
+    assert b.step == 2000
+
+
+# ------------------------------------------------------------------ full size, bench launch configuration
+
+def test_config3_full_grid_sampled_parity(aw, orc):
+    """BASELINE configs[3] at full size (2048 x 2048, the launch configuration bench.py times), short
+    horizon; sampled trajectories (every 256th row/column + 1024 hashed pixels) against the oracle."""
+    cfg = aw.CONFIGS[3]
+    ens = aw.Ensemble(cfg["gx"] * cfg["gy"], tangent=True, wind=True)
+    aw.aw_init_shell(ens, grid_from_cfg(aw, cfg), cfg["E"], cfg["eps"], cfg["seed"])
+    n = ens.n
+    G = cfg["gx"]
+    rows = np.arange(0, G, 256)
+    lattice = (rows[:, None] * G + rows[None, :]).ravel()
+    hashed = np.array([orc.mix64(3, i) % n for i in range(1024)], dtype=np.int64)
+    corner = np.array([0, 1, G - 1, n - 1, n - G, G * 3 + 5])      # includes off-shell corner pixels
+    sample = np.unique(np.concatenate([lattice, hashed, corner]))
+    st = ensemble_to_oracle(ens, orc)
+    assert (st.status == 0).sum() > 0 and (st.status == 0).sum() < 0.01 * n
+    aw.aw_integrate(ens, n, 1000, cfg["dt"], cfg["stride"])
+    for k in sample:
+        orc.integrate(st, 1000, cfg["dt"], cfg["stride"], k0=int(k), k1=int(k) + 1, advance_clock=False)
+    got = ensemble_to_oracle(ens, orc)
+    assert np.array_equal(got.status[sample], st.status[sample])
+    live = st.status[sample] == 1
+    thr = math.log(1000 * cfg["dt"]) + 3.0
+    regular = live & (st.acc[1, sample] <= thr)
+    err = state_rel_err(got.q[:, sample], got.wind[:, sample], st.q[:, sample], st.wind[:, sample], regular)
+    assert err.max() <= 1e-10, err.max()
+    assert np.max(np.abs(got.acc[1, sample][regular] - st.acc[1, sample][regular])) <= 1e-5
+    # properties at full size: shell layer and bounded energy error for every live trajectory
+    livef = got.status == 1
+    P2 = np.sum(got.q[3:, :n][:, livef] ** 2, axis=0)
+    dH = got.acc[3, :n][livef]
+    assert dH.max() < 1e-9
+    assert np.all(P2 >= 2 * (1 - 2 * cfg["eps"]) - 2 * dH.max()) and np.all(P2 <= 2 * (1 + 2 * cfg["eps"]) + 2 * dH.max())
+    fli = aw.aw_indicator(ens, aw.AW_IND_FLI).cpu().numpy()
+    assert np.isnan(fli[~livef]).all() and np.isfinite(fli[livef]).all()
