@@ -14,8 +14,9 @@ collective except the histogram sum).
 
 value   = live trajectory-steps / s, whole job, inputs resident in HBM (device-timed, max over ranks)
 e2e     = same metric through aw_map_host: host (pinned) state in, image + histogram out, copies timed
-roofline= fp64 ALU bound: nominal flops (498 / traj-step for order 4 with tangent) per
-          integrate launch / its CUDA-event duration, against 148 SM x 64 DFMA/clk x 2 x 1.965 GHz
+roofline= fp64 ALU bound: min(nominal 498 flop / traj-step for order 4 with tangent; fp64
+          flops the step loop's SASS executes) per integrate launch / its CUDA-event duration, against
+          148 SM x 64 DFMA/clk x 2 x 1.965 GHz
 cpu_baseline = the oracle (oracle/aw_oracle.cpp, as it stands) on the host cores, bounded sample
 --impl reference = the oracle as the reference arm (rank 0 only).
 """
@@ -249,19 +250,33 @@ def run_ours(args, cfg, order, tangent):
     live_all = int(livet.item())
     value = live_all * horizon * args.steps / (total_ms * 1e-3)
 
-    # dominant kernel: integrate_kernel — average launch duration from CUDA events on its stream
+    # dominant kernel: integrate_kernel — average launch duration from CUDA events on its stream.
+    # flops per trajectory-step = min(nominal accounting figure, fp64 flops the SASS of the step loop
+    # executes) so neither a fat nor a lean sincos can inflate the fraction.
+    from paper_1107_4107_b200 import sass_count
     integ_ms = sum(a.elapsed_time(b) for a, b in integ_events)
     n_integ_launches = args.steps * math.ceil(horizon / (20000 // cfg["stride"] * cfg["stride"]))
-    flops_per_step = NOMINAL_FLOPS[(order, tangent)]
+    level = aw.aw_trig_level(ens, cfg["dt"])
+    mix = sass_count.integrate_step_mix(order, tangent, level)
+    flops_nominal = NOMINAL_FLOPS[(order, tangent)]
+    flops_per_step = min(flops_nominal, mix["flops"])
     launch_ms = integ_ms / n_integ_launches
     steps_per_launch = horizon * args.steps / n_integ_launches
-    achieved = live * steps_per_launch * flops_per_step / (launch_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "integrate_kernel<%d,%s>" % (3 if order == 4 else 7, str(tangent).lower()),
+    kernel_rate = live * steps_per_launch / (launch_ms * 1e-3)          # traj-steps/s inside the kernel
+    achieved = kernel_rate * flops_per_step / 1e12
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    fp64_slots = sms * 64 * 1.965e9                                      # fp64 thread-instructions / s
+    roofline = {"bound": "alu",
+                "kernel": "integrate_kernel<%d,%s,%d>" % (3 if order == 4 else 7, str(tangent).lower(), level),
                 "achieved": achieved, "peak": FP64_PEAK_TFLOPS_NOMINAL, "unit": "TFLOP/s",
                 "frac": achieved / FP64_PEAK_TFLOPS_NOMINAL, "traffic": None,
-                "peak_source": "derived: 148 SM x 64 DFMA/clk/SM x 2 flop x 1.965 GHz (DESIGN.md §8); "
+                "peak_source": "derived: 148 SM x 64 DFMA/clk/SM x 2 flop x 1.965 GHz (DESIGN.md §6.1); "
                                "MEASURED_PEAKS.json has no fp64 entry",
-                "flops_per_traj_step_nominal": flops_per_step,
+                "flops_per_traj_step": flops_per_step, "flops_per_traj_step_nominal": flops_nominal,
+                "flops_per_traj_step_executed": mix["flops"],
+                "sass_per_step": {k: mix[k] for k in ("dfma", "dmul", "dadd", "other")},
+                "fp64_pipe_busy_est": kernel_rate * (mix["dfma"] + mix["dmul"] + mix["dadd"]) / fp64_slots,
+                "trig_level": level,
                 "launch_ms": launch_ms, "launches_timed": n_integ_launches,
                 "kernel_share_of_step": integ_ms / total_ms}
 
@@ -280,7 +295,6 @@ def run_ours(args, cfg, order, tangent):
     # measured DFMA peak beside the derived one (rank 0; independent chains, all SMs)
     if rank == 0:
         try:
-            sms = torch.cuda.get_device_properties(dev).multi_processor_count
             best = 0.0
             for chains in (8, 16):
                 msd, cnt = aw.aw_dfma_peak_probe(sms * 8, 256, chains, 1 << 16, device=dev)

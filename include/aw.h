@@ -83,6 +83,9 @@ typedef struct {
   int64_t step;    /* elapsed steps                                                           */
   int32_t order;   /* 4 or 6 (R1); set by the caller before aw_integrate; default 4           */
   int32_t ready;   /* set to 1 by aw_init_shell (or by the caller after uploading a state)    */
+  int32_t trig;    /* 0 (default): running (sin, cos) pairs advanced by rotations, see aw_integrate;
+                      1: evaluate the device sincos at every stage                            */
+  int32_t reserved; /* must be 0                                                              */
   void *stream;    /* cudaStream_t; NULL = legacy default stream                              */
 } aw_state;
 
@@ -129,6 +132,13 @@ AW_API int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps,
  * backwards).  steps == 0 or n == 0 is a no-op.  AW_ERANGE if stride*|dt|*sqrt(2(E+2|eps|)) >= 1024
  * (the angle would leave the range the two-constant argument reduction handles exactly, R7).
  * AW_ESTATE if !s->ready or order not in {4, 6}.  Advances s->t and s->step.
+ * Trigonometry: the kick needs sin/cos of x, y and 2z at every stage.  With s->trig == 0 the kernel
+ * carries the three (sin, cos) pairs in registers and advances them through each drift by a rotation
+ * with the drift angle d = a_s p (Taylor polynomials in d; the degree is picked on the host from
+ * max_s |a_s| sqrt(2(E + 2|eps|)) so the truncation stays below 2^-60; aw_trig_level reports it), and
+ * recomputes them from the angles with the device sincos at every checkpoint and at least every 128
+ * steps.  s->E must therefore bound the energy of an uploaded state.  If the drift angle can exceed
+ * 0.0708 rad, or with s->trig == 1, the device sincos is evaluated at every stage instead (level 0).
  * The work is split into kernel launches of at most AW_MAX_STEPS_PER_LAUNCH steps (a multiple of
  * stride); the result does not depend on the split. */
 #define AW_MAX_STEPS_PER_LAUNCH 20000
@@ -154,6 +164,10 @@ AW_API int aw_density(const aw_state *s, uint32_t *hist_dev, int32_t gx, int32_t
  * order 6) or AW_EINVAL.  Order-6 weights are obtained inside the library by Newton iteration on the
  * four order conditions in extended precision. */
 AW_API int aw_stage_constants(int order, double dt, double eps, double *a_host, double *b_host);
+/* Trigonometry level aw_integrate would use for this state and dt: 0 = device sincos at every stage,
+ * 1..4 = running pairs with Taylor degrees (x/y pair, 2z pair) = (3,3), (3,4), (4,4), (4,5); or a
+ * negative aw_status.  Pure host arithmetic. */
+AW_API int aw_trig_level(const aw_state *s, double dt);
 /* The common tangent vector of tangent_mode 0: unit vector from u(seed, 2^63-1, 5..10) (R12). */
 AW_API int aw_common_tangent(uint64_t seed, double *t6_host);
 

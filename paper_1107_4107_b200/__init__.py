@@ -9,7 +9,7 @@ from .binding import (AW_IND_CLASS, AW_IND_DH, AW_IND_FLI, AW_IND_FTLE, AwError,
                       aw_common_tangent, aw_density, aw_dfma_peak_probe, aw_hamiltonian_probe,
                       aw_indicator, aw_init_shell, aw_integrate, aw_launch_count, aw_map_host,
                       aw_sincos_probe, aw_stage_constants, aw_state_bytes, aw_strerror,
-                      aw_uniform_probe, aw_version, lib, make_grid)
+                      aw_trig_level, aw_uniform_probe, aw_version, lib, make_grid)
 from .configs import CONFIGS
 
 __all__ = [n for n in dir() if n.startswith(("aw_", "AW_")) or n in

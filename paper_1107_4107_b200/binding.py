@@ -30,7 +30,8 @@ class AwState(C.Structure):
                 ("q", C.c_void_p), ("w", C.c_void_p), ("acc", C.c_void_p), ("wind", C.c_void_p),
                 ("status", C.c_void_p),
                 ("E", C.c_double), ("eps", C.c_double), ("t", C.c_double), ("step", C.c_int64),
-                ("order", C.c_int32), ("ready", C.c_int32), ("stream", C.c_void_p)]
+                ("order", C.c_int32), ("ready", C.c_int32), ("trig", C.c_int32), ("reserved", C.c_int32),
+                ("stream", C.c_void_p)]
 
 
 class Grid(C.Structure):
@@ -82,6 +83,7 @@ def lib():
         L.aw_density.argtypes = [C.POINTER(AwState), vp, i32, i32, dbl, dbl, C.c_int, vp]
         L.aw_stage_constants.argtypes = [C.c_int, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
         L.aw_common_tangent.argtypes = [u64, C.POINTER(dbl)]
+        L.aw_trig_level.argtypes = [C.POINTER(AwState), dbl]
         L.aw_map_host.argtypes = [C.POINTER(AwState), C.POINTER(HostIn), i64, dbl, i64, C.c_int, dbl,
                                   i32, i32, dbl, dbl, vp, vp, C.POINTER(HostOut)]
         L.aw_sincos_probe.argtypes = [vp, i64, vp, vp, vp]
@@ -135,6 +137,10 @@ def aw_stage_constants(order, dt, eps):
     return list(a[:S + 1]), list(b[:S])
 
 
+def aw_trig_level(ens, dt):
+    return _check(lib().aw_trig_level(C.byref(ens.c), dt), "aw_trig_level")
+
+
 def aw_common_tangent(seed):
     t = (C.c_double * 6)()
     _check(lib().aw_common_tangent(seed, t), "aw_common_tangent")
@@ -158,7 +164,7 @@ class Ensemble:
         self.status = torch.zeros((max(n, 1),), dtype=torch.uint8, device=dev)
         self.c = AwState(n, pitch, self.q.data_ptr(), self.w.data_ptr() if tangent else None,
                          self.acc.data_ptr(), self.wind.data_ptr() if wind else None,
-                         self.status.data_ptr(), float("nan"), float("nan"), 0.0, 0, order, 0, None)
+                         self.status.data_ptr(), float("nan"), float("nan"), 0.0, 0, order, 0, 0, 0, None)
 
     # plain-data views of the struct
     E = property(lambda s: s.c.E)
@@ -173,6 +179,14 @@ class Ensemble:
     @order.setter
     def order(self, v):
         self.c.order = v
+
+    @property
+    def trig(self):
+        return self.c.trig
+
+    @trig.setter
+    def trig(self, v):
+        self.c.trig = v
 
     def bind_stream(self, stream=None):
         self.c.stream = _stream_ptr(stream)

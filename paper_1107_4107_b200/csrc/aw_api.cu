@@ -198,6 +198,17 @@ int aw_stage_constants(int order, double dt, double eps, double *a_host, double 
   return S;
 }
 
+int aw_trig_level(const aw_state *s, double dt) {
+  if (!s || !(dt != 0.0) || !std::isfinite(dt)) return AW_EINVAL;
+  if (!std::isfinite(s->E) || !std::isfinite(s->eps) || (s->order != 4 && s->order != 6)) return AW_ESTATE;
+  if (s->trig) return 0;
+  double a[kMaxStages + 1], b[kMaxStages];
+  const int S = stage_constants(s->order, dt, s->eps, a, b);
+  double amax = std::fmax(std::fabs(a[0]), std::fmax(std::fabs(a[S]), std::fabs(a[S] + a[0])));
+  for (int k = 1; k < S; ++k) amax = std::fmax(amax, std::fabs(a[k]));
+  return trig_level_for(amax * std::sqrt(2.0 * (s->E + 2.0 * std::fabs(s->eps))));
+}
+
 int aw_common_tangent(uint64_t seed, double *t6_host) {
   if (!t6_host) return AW_EINVAL;
   common_tangent(seed, t6_host);
@@ -262,8 +273,17 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
   p.a_last = a[S];
   p.a_merge = a[S] + a[0];
   for (int k = 1; k < S; ++k) p.a_mid[k - 1] = a[k];
-  for (int k = 0; k < S; ++k) { p.b2[k] = 2.0 * b[k]; p.b4[k] = 4.0 * b[k]; }
+  for (int k = 0; k < S; ++k) { p.b1[k] = b[k]; p.b2[k] = 2.0 * b[k]; p.b4[k] = 4.0 * b[k]; }
+  p.a2_first = 2.0 * p.a_first; p.a2_merge = 2.0 * p.a_merge; p.a2_last = 2.0 * p.a_last;
+  for (int k = 0; k < kMaxStages; ++k) p.a2_mid[k] = 2.0 * p.a_mid[k];
   p.eps = s->eps;
+  // running-(sin, cos) variant: degree from the largest drift angle, re-synchronisation cadence from stride
+  double amax = std::fabs(p.a_first);
+  amax = std::fmax(amax, std::fmax(std::fabs(p.a_merge), std::fabs(p.a_last)));
+  for (int k = 0; k + 1 < S; ++k) amax = std::fmax(amax, std::fabs(p.a_mid[k]));
+  p.level = s->trig ? 0 : trig_level_for(amax * vmax);
+  const int64_t pieces = (stride + kMaxChunk - 1) / kMaxChunk;
+  p.chunk = (int32_t)((stride + pieces - 1) / pieces);
 
   const int64_t total_chk = steps / stride;
   int64_t chk_per_launch = AW_MAX_STEPS_PER_LAUNCH / stride;

@@ -1,16 +1,26 @@
 // aw_integrate.cu — §8(a) a2 + a3 + a4: the integrator kernel.
 //
-// One trajectory per thread ("complete parallelisation"), the six state words and the six tangent
-// words live in registers for the whole launch; HBM is touched at launch start and end, plus one
-// read-modify-write of the accumulator planes per checkpoint.  The stage loop is fully unrolled so
-// a_s, 2b_s, 4b_s are constant-bank operands.  Bound by the fp64 pipe: per stage 3 sincos (57 fp64
-// instructions) + 3 drift + 11 kick (+ 3 + 16 with the tangent map).
+// One trajectory per thread ("complete parallelisation"); the six state words, the six tangent
+// words and the running (sin, cos) pairs live in registers for the whole launch; HBM is touched at launch
+// start and end, plus one read-modify-write of the accumulator planes per checkpoint.  The stage loop is
+// fully unrolled so a_s, b_s, 2b_s, 4b_s are constant-bank operands.  Bound by the fp64 pipe.
 //
 // Scheme (ref. 25; R2): for s = 1..S { X += a_s P ; P -= b_s grad H_p(X) }  X += a_{S+1} P.
 // Inside a block of `stride` steps the closing drift of a step and the opening drift of the next are
 // one FMA with the constant a_{S+1} + a_1 (same map, one rounding fewer; DESIGN.md §7 D3).
-// Model (eq. 2) with u = cos^2 z, d = sin z cos z:  H_p = 2 cx cy u,
-//   grad H_p = (-2 sx cy u, -2 cx sy u, -4 cx cy d),  Hessian in SURVEY.md Appendix A.2.
+// Model (eq. 2) with F = 1 + cos 2z:  H_p = cx cy F,
+//   grad H_p = (-sx cy F, -cx sy F, -2 cx cy sin 2z),  Hessian in SURVEY.md Appendix A.2.
+//
+// Trigonometry.  LEVEL 0: the device sincos (aw_trig.cuh) of x, y, z at every stage.
+// LEVEL >= 1: the pairs (sin x, cos x), (sin y, cos y), (sin 2z, cos 2z) are carried in registers and
+// advanced through every drift X += a P by the rotation with the drift angle d = a p (2 a pz for 2z):
+//     s' = s + (s m + c g),  c' = c + (c m - s g),   g = sin d,  m = cos d - 1,
+// g and m being Taylor polynomials in d whose degree the host picks from the largest possible |d| so
+// that the truncation error stays below 2^-60 (trig_level_for).  The pairs are re-synchronised from the
+// tracked angles with the full sincos at every checkpoint and at least every kMaxChunk steps, which
+// bounds the rounding random walk of the rotations at a few 1e-15.
+#include <cmath>
+
 #include "aw_internal.cuh"
 #include "aw_model.cuh"
 #include "aw_trig.cuh"
@@ -36,7 +46,101 @@ __device__ __forceinline__ double wrap_angle(double x, int &turns) {
   return fma(-k, kTwoPiLo, fma(-k, kTwoPiHi, x));
 }
 
-template <int S, bool TAN>
+// g = sin d, m = cos d - 1 for a small angle d: Taylor series with N terms beyond the leading one.
+// Truncation: |d|^(2N+3)/(2N+3)! in g, |d|^(2N+2)/(2N+2)! in m.  N + N FMA + 3 DMUL.
+template <int N>
+__device__ __forceinline__ void small_sincos(double d, double &g, double &m) {
+  constexpr double S[5] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0, -1.0 / 39916800.0};
+  constexpr double C[5] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0, -1.0 / 3628800.0};
+  static_assert(N >= 1 && N <= 5, "degree");
+  const double z = d * d;
+  double ps = S[N - 1], pc = C[N - 1];
+#pragma unroll
+  for (int i = N - 2; i >= 0; --i) {
+    ps = fma(ps, z, S[i]);
+    pc = fma(pc, z, C[i]);
+  }
+  g = fma(d * z, ps, d);
+  m = z * pc;
+}
+
+// (s, c) <- rotation of (s, c) by the angle whose sine is g and cosine is 1 + m; <= 1 ulp each.
+__device__ __forceinline__ void rotate(double &s, double &c, double g, double m) {
+  const double s1 = fma(c, g, fma(s, m, s));
+  const double c1 = fma(-s, g, fma(c, m, c));
+  s = s1;
+  c = c1;
+}
+
+// Degrees (x/y pair, 2z pair) of the trigonometry levels; the angle of the 2z pair is twice as large.
+template <int LEVEL> struct Deg;
+template <> struct Deg<0> { static constexpr int xy = 1, z = 1; };  // unused
+template <> struct Deg<1> { static constexpr int xy = 3, z = 3; };
+template <> struct Deg<2> { static constexpr int xy = 3, z = 4; };
+template <> struct Deg<3> { static constexpr int xy = 4, z = 4; };
+template <> struct Deg<4> { static constexpr int xy = 4, z = 5; };
+
+// Everything a thread carries between stages.
+template <bool TAN>
+struct Traj {
+  double x, y, z, px, py, pz;
+  double dx, dy, dz, dpx, dpy, dpz;
+  double sx, cx, sy, cy, s2, c2;  // sin x, cos x, sin y, cos y, sin 2z, cos 2z (LEVEL >= 1)
+};
+
+template <bool TAN, int LEVEL>
+__device__ __forceinline__ void drift(Traj<TAN> &t, double a, double a2) {
+  if (LEVEL > 0) {
+    double g, m;
+    small_sincos<Deg<LEVEL>::xy>(a * t.px, g, m);
+    rotate(t.sx, t.cx, g, m);
+    small_sincos<Deg<LEVEL>::xy>(a * t.py, g, m);
+    rotate(t.sy, t.cy, g, m);
+    small_sincos<Deg<LEVEL>::z>(a2 * t.pz, g, m);
+    rotate(t.s2, t.c2, g, m);
+  }
+  t.x = fma(a, t.px, t.x); t.y = fma(a, t.py, t.y); t.z = fma(a, t.pz, t.z);
+  if (TAN) { t.dx = fma(a, t.dpx, t.dx); t.dy = fma(a, t.dpy, t.dy); t.dz = fma(a, t.dpz, t.dz); }
+}
+
+template <bool TAN, int LEVEL>
+__device__ __forceinline__ void resync(Traj<TAN> &t) {
+  if (LEVEL > 0) {
+    sincos(t.x, t.sx, t.cx);
+    sincos(t.y, t.sy, t.cy);
+    sincos(2.0 * t.z, t.s2, t.c2);
+  }
+}
+
+// kick of stage s: P -= b grad H_p(X), dP -= b Hess H_p(X) dX (R3), b1 = b, b2 = 2b, b4 = 4b
+template <bool TAN, int LEVEL>
+__device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2, double b4) {
+  if (LEVEL == 0) {
+    double sz, cz;
+    sincos(t.x, t.sx, t.cx);
+    sincos(t.y, t.sy, t.cy);
+    sincos(t.z, sz, cz);
+    t.c2 = fma(cz + cz, cz, -1.0);  // cos 2z = 2 cz^2 - 1
+    t.s2 = (sz + sz) * cz;          // sin 2z
+  }
+  const double F = fma(b1, t.c2, b1);  // b (1 + cos 2z)
+  const double G = b2 * t.s2;          // 2 b sin 2z
+  const double c = t.cx * t.cy, sc = t.sx * t.cy, cs = t.cx * t.sy;
+  t.px = fma(sc, F, t.px);
+  t.py = fma(cs, F, t.py);
+  t.pz = fma(c, G, t.pz);
+  if (TAN) {
+    // rows of -b Hess H_p: (e1,-e2,-e3), (-e2,e1,-e4), (-e3,-e4,e5)
+    const double ss = t.sx * t.sy;
+    const double e1 = c * F, e2 = ss * F, e3 = sc * G, e4 = cs * G;
+    const double e5 = c * (b4 * t.c2);  // 4 b cx cy cos 2z
+    t.dpx = fma(e1, t.dx, t.dpx); t.dpx = fma(-e2, t.dy, t.dpx); t.dpx = fma(-e3, t.dz, t.dpx);
+    t.dpy = fma(e1, t.dy, t.dpy); t.dpy = fma(-e2, t.dx, t.dpy); t.dpy = fma(-e4, t.dz, t.dpy);
+    t.dpz = fma(e5, t.dz, t.dpz); t.dpz = fma(-e3, t.dx, t.dpz); t.dpz = fma(-e4, t.dy, t.dpz);
+  }
+}
+
+template <int S, bool TAN, int LEVEL>
 __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS)
     integrate_kernel(const __grid_constant__ IntegrateParams p) {
   const int64_t k = (int64_t)blockIdx.x * AW_BLOCK + threadIdx.x;
@@ -44,105 +148,112 @@ __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS)
   if (p.status[k] != AW_ST_LIVE) return;
   const int64_t P = p.pitch;
 
-  double x = p.q[k], y = p.q[P + k], z = p.q[2 * P + k];
-  double px = p.q[3 * P + k], py = p.q[4 * P + k], pz = p.q[5 * P + k];
-  double dx = 0, dy = 0, dz = 0, dpx = 0, dpy = 0, dpz = 0;
+  Traj<TAN> t;
+  t.x = p.q[k]; t.y = p.q[P + k]; t.z = p.q[2 * P + k];
+  t.px = p.q[3 * P + k]; t.py = p.q[4 * P + k]; t.pz = p.q[5 * P + k];
   if (TAN) {
-    dx = p.w[k]; dy = p.w[P + k]; dz = p.w[2 * P + k];
-    dpx = p.w[3 * P + k]; dpy = p.w[4 * P + k]; dpz = p.w[5 * P + k];
+    t.dx = p.w[k]; t.dy = p.w[P + k]; t.dz = p.w[2 * P + k];
+    t.dpx = p.w[3 * P + k]; t.dpy = p.w[4 * P + k]; t.dpz = p.w[5 * P + k];
   }
+  resync<TAN, LEVEL>(t);
   int status = AW_ST_LIVE;
 
   for (int chk = 0; chk < p.nchk; ++chk) {
-    // opening drift of the block
-    x = fma(p.a_first, px, x); y = fma(p.a_first, py, y); z = fma(p.a_first, pz, z);
-    if (TAN) { dx = fma(p.a_first, dpx, dx); dy = fma(p.a_first, dpy, dy); dz = fma(p.a_first, dpz, dz); }
+    drift<TAN, LEVEL>(t, p.a_first, p.a2_first);  // opening drift of the block
 
 #pragma unroll 1
-    for (int i = p.stride; i > 0; --i) {
+    for (int rem = p.stride; rem > 0;) {
+      const int m = rem < p.chunk ? rem : p.chunk;
+      rem -= m;
+#pragma unroll 1
+      for (int i = m; i > 0; --i) {
 #pragma unroll
-      for (int s = 0; s < S; ++s) {
-        double sx, cx, sy, cy, sz, cz;
-        sincos(x, sx, cx);
-        sincos(y, sy, cy);
-        sincos(z, sz, cz);
-        const double u = cz * cz, d = sz * cz;
-        const double U = p.b2[s] * u;  // 2 b u
-        const double D = p.b4[s] * d;  // 4 b d
-        const double c = cx * cy, sc = sx * cy, cs = cx * sy;
-        // kick: P -= b grad H_p
-        px = fma(sc, U, px);
-        py = fma(cs, U, py);
-        pz = fma(c, D, pz);
-        if (TAN) {
-          // tangent kick: dP -= b Hess H_p dX, rows (e1,-e2,-e3), (-e2,e1,-e4), (-e3,-e4,e5)
-          const double ss = sx * sy;
-          const double e1 = c * U, e2 = ss * U, e3 = sc * D, e4 = cs * D;
-          const double e5 = c * fma(4.0, U, -p.b4[s]);  // 4 b c (2u - 1)
-          dpx = fma(e1, dx, dpx); dpx = fma(-e2, dy, dpx); dpx = fma(-e3, dz, dpx);
-          dpy = fma(e1, dy, dpy); dpy = fma(-e2, dx, dpy); dpy = fma(-e4, dz, dpy);
-          dpz = fma(e5, dz, dpz); dpz = fma(-e3, dx, dpz); dpz = fma(-e4, dy, dpz);
+        for (int s = 0; s < S; ++s) {
+          kick<TAN, LEVEL>(t, p.b1[s], p.b2[s], p.b4[s]);
+          if (s < S - 1) drift<TAN, LEVEL>(t, p.a_mid[s], p.a2_mid[s]);
         }
-        if (s < S - 1) {
-          const double a = p.a_mid[s];
-          x = fma(a, px, x); y = fma(a, py, y); z = fma(a, pz, z);
-          if (TAN) { dx = fma(a, dpx, dx); dy = fma(a, dpy, dy); dz = fma(a, dpz, dz); }
-        }
+        const bool last = (i == 1) && (rem == 0);
+        drift<TAN, LEVEL>(t, last ? p.a_last : p.a_merge, last ? p.a2_last : p.a2_merge);
       }
-      const double a = (i == 1) ? p.a_last : p.a_merge;
-      x = fma(a, px, x); y = fma(a, py, y); z = fma(a, pz, z);
-      if (TAN) { dx = fma(a, dpx, dx); dy = fma(a, dpy, dy); dz = fma(a, dpz, dz); }
+      if (rem > 0) resync<TAN, LEVEL>(t);
     }
 
     // ---- fused checkpoint (R4): (i) renormalise + log growth, (ii) energy error, (iii) wrap
     bool finite = true;
     if (TAN) {
-      double s2 = dx * dx;
-      s2 = fma(dy, dy, s2); s2 = fma(dz, dz, s2);
-      s2 = fma(dpx, dpx, s2); s2 = fma(dpy, dpy, s2); s2 = fma(dpz, dpz, s2);
+      double s2 = t.dx * t.dx;
+      s2 = fma(t.dy, t.dy, s2); s2 = fma(t.dz, t.dz, s2);
+      s2 = fma(t.dpx, t.dpx, s2); s2 = fma(t.dpy, t.dpy, s2); s2 = fma(t.dpz, t.dpz, s2);
       const double nu = sqrt(s2);
       const double inv = 1.0 / nu;
-      dx *= inv; dy *= inv; dz *= inv; dpx *= inv; dpy *= inv; dpz *= inv;
+      t.dx *= inv; t.dy *= inv; t.dz *= inv; t.dpx *= inv; t.dpy *= inv; t.dpz *= inv;
       const double logsum = p.acc[k] + log(nu);
       p.acc[k] = logsum;
       if (logsum > p.acc[P + k]) p.acc[P + k] = logsum;
-      finite = isfinite(dx) && isfinite(dy) && isfinite(dz) && isfinite(dpx) && isfinite(dpy) &&
-               isfinite(dpz);
+      finite = isfinite(t.dx) && isfinite(t.dy) && isfinite(t.dz) && isfinite(t.dpx) && isfinite(t.dpy) &&
+               isfinite(t.dpz);
     }
-    const double dH = fabs(hamiltonian_dev(x, y, z, px, py, pz, p.eps) - p.acc[2 * P + k]);
+    const double dH = fabs(hamiltonian_dev(t.x, t.y, t.z, t.px, t.py, t.pz, p.eps) - p.acc[2 * P + k]);
     if (dH > p.acc[3 * P + k]) p.acc[3 * P + k] = dH;
     int tx, ty, tz;
-    x = wrap_angle(x, tx); y = wrap_angle(y, ty); z = wrap_angle(z, tz);
+    t.x = wrap_angle(t.x, tx); t.y = wrap_angle(t.y, ty); t.z = wrap_angle(t.z, tz);
     if (p.wind) {
       p.wind[k] += tx; p.wind[P + k] += ty; p.wind[2 * P + k] += tz;
     }
-    finite = finite && isfinite(x) && isfinite(y) && isfinite(z) && isfinite(px) && isfinite(py) &&
-             isfinite(pz);
+    finite = finite && isfinite(t.x) && isfinite(t.y) && isfinite(t.z) && isfinite(t.px) && isfinite(t.py) &&
+             isfinite(t.pz);
     if (!finite) { status = AW_ST_NONFINITE; break; }
+    resync<TAN, LEVEL>(t);  // from the wrapped angles: the same values a new launch would start from
   }
 
-  p.q[k] = x; p.q[P + k] = y; p.q[2 * P + k] = z;
-  p.q[3 * P + k] = px; p.q[4 * P + k] = py; p.q[5 * P + k] = pz;
+  p.q[k] = t.x; p.q[P + k] = t.y; p.q[2 * P + k] = t.z;
+  p.q[3 * P + k] = t.px; p.q[4 * P + k] = t.py; p.q[5 * P + k] = t.pz;
   if (TAN) {
-    p.w[k] = dx; p.w[P + k] = dy; p.w[2 * P + k] = dz;
-    p.w[3 * P + k] = dpx; p.w[4 * P + k] = dpy; p.w[5 * P + k] = dpz;
+    p.w[k] = t.dx; p.w[P + k] = t.dy; p.w[2 * P + k] = t.dz;
+    p.w[3 * P + k] = t.dpx; p.w[4 * P + k] = t.dpy; p.w[5 * P + k] = t.dpz;
   }
   if (status != AW_ST_LIVE) p.status[k] = (uint8_t)status;
 }
 
-template <int S, bool TAN>
+template <int S, bool TAN, int LEVEL>
 cudaError_t launch_one(const IntegrateParams &p, cudaStream_t st) {
   const int64_t blocks = (p.n + AW_BLOCK - 1) / AW_BLOCK;
-  integrate_kernel<S, TAN><<<(unsigned)blocks, AW_BLOCK, 0, st>>>(p);
+  integrate_kernel<S, TAN, LEVEL><<<(unsigned)blocks, AW_BLOCK, 0, st>>>(p);
   count_launch();
   return cudaGetLastError();
 }
 
+template <int S, bool TAN>
+cudaError_t launch_level(const IntegrateParams &p, cudaStream_t st) {
+  switch (p.level) {
+    case 1: return launch_one<S, TAN, 1>(p, st);
+    case 2: return launch_one<S, TAN, 2>(p, st);
+    case 3: return launch_one<S, TAN, 3>(p, st);
+    case 4: return launch_one<S, TAN, 4>(p, st);
+    default: return launch_one<S, TAN, 0>(p, st);
+  }
+}
+
 }  // namespace
 
+// Largest |d| each level may see on the x/y pairs (the 2z pair sees 2|d|) with both Taylor truncations
+// below 2^-60 ~ 8.7e-19 (they are systematic, so 300 of them still sum to < 3e-16):
+//   m of degree N truncates at |d|^(2N+2)/(2N+2)!, g at |d|^(2N+3)/(2N+3)!:
+//   N = 3: |d| <= 0.0208 (m), 0.0408 (g);  N = 4: 0.0708, 0.112;  N = 5: 0.165, 0.23.
+// level 1 = (3,3): 2|d| <= 0.0208;  level 2 = (3,4): |d| <= 0.0208;  level 3 = (4,4): 2|d| <= 0.0708;
+// level 4 = (4,5): |d| <= 0.0708;  beyond: level 0 (full sincos every stage).
+int trig_level_for(double d) {
+  if (!(d == d)) return 0;
+  if (d <= 0.0104) return 1;
+  if (d <= 0.0208) return 2;
+  if (d <= 0.0354) return 3;
+  if (d <= 0.0708) return 4;
+  return 0;
+}
+
 cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, cudaStream_t st) {
-  if (order == 4) return tangent ? launch_one<3, true>(p, st) : launch_one<3, false>(p, st);
-  return tangent ? launch_one<7, true>(p, st) : launch_one<7, false>(p, st);
+  if (order == 4) return tangent ? launch_level<3, true>(p, st) : launch_level<3, false>(p, st);
+  return tangent ? launch_level<7, true>(p, st) : launch_level<7, false>(p, st);
 }
 
 __global__ void hamiltonian_probe_kernel(const double *q, int64_t n, int64_t P, double eps, double *out) {

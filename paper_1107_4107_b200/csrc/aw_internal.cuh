@@ -20,10 +20,15 @@ struct IntegrateParams {
   int64_t n, pitch;
   int32_t nchk;    // checkpoints in this launch
   int32_t stride;  // steps between checkpoints
+  int32_t chunk;   // steps between re-synchronisations of the running (sin, cos) pairs; divides the
+                   // stride into equal-as-possible pieces of <= kMaxChunk steps (a function of stride only)
+  int32_t level;   // trigonometry variant picked on the host from the largest drift angle (aw_integrate.cu)
   double a_first;  // a_1: drift that opens a block of `stride` steps
   double a_merge;  // a_{S+1} + a_1: closing drift of one step merged with the opening drift of the next
   double a_last;   // a_{S+1}: drift that closes the block
   double a_mid[kMaxStages];  // a_2 .. a_S (drift after kick s, s = 1..S-1); a_mid[S-1] unused
+  double a2_first, a2_merge, a2_last, a2_mid[kMaxStages];  // twice the above (exact): drift of the angle 2z
+  double b1[kMaxStages];     // b_s
   double b2[kMaxStages];     // 2 b_s
   double b4[kMaxStages];     // 4 b_s
   double eps;
@@ -44,6 +49,9 @@ struct InitParams {
 
 // host-side launchers (each returns cudaError_t of the launch and bumps the launch counter)
 cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, cudaStream_t st);
+// Trigonometry variant for a largest drift angle max_s |a_s| * max|p| (0 = full sincos every stage).
+int trig_level_for(double max_drift_angle);
+constexpr int kMaxChunk = 128;
 cudaError_t launch_init(const InitParams &p, cudaStream_t st);
 cudaError_t launch_indicator(const double *acc, const uint8_t *status, int64_t n, int64_t pitch, int kind,
                              double thr, double t, void *out, cudaStream_t st);

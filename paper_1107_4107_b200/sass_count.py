@@ -1,0 +1,61 @@
+"""Count the fp64 instructions one trajectory-step executes, from the SASS of the built library.
+
+bench.py's reporting rule: flop/s = traj-steps/s x min(nominal, executed) flops per step,
+so the roofline fraction cannot be inflated by the accounting convention.  "Executed" is read here from
+`cuobjdump -sass libaw.so`: the innermost loop of integrate_kernel<S, TAN, LEVEL> is exactly one step
+(all stages unrolled), so its DFMA / DMUL / DADD counts are the per-step counts (checkpoint and
+re-synchronisation code, < 1 % at stride 100, is outside that loop and not counted).
+
+    python -m paper_1107_4107_b200.sass_count          # table for every instantiation
+"""
+import collections
+import os
+import re
+import subprocess
+
+from .build import LIB
+
+_cache = {}
+
+
+def _functions(lib):
+    out = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True, check=True).stdout
+    for chunk in re.split(r"\n\s*Function : ", out)[1:]:
+        yield chunk.split("\n", 1)[0].strip(), chunk
+
+
+def integrate_step_mix(order, tangent, level, lib=LIB):
+    """{'dfma', 'dmul', 'dadd', 'other', 'flops'} per trajectory-step of integrate_kernel<S,TAN,LEVEL>."""
+    key = (os.path.getmtime(lib), order, bool(tangent), level)
+    if key in _cache:
+        return _cache[key]
+    tag = "integrate_kernelILi%dELb%dELi%dE" % (3 if order == 4 else 7, 1 if tangent else 0, level)
+    for name, text in _functions(lib):
+        if tag not in name:
+            continue
+        ins = [(int(m.group(1), 16), m.group(2)) for m in
+               re.finditer(r"/\*([0-9a-f]{4,6})\*/\s+([^;]*);", text)]
+        loops = []
+        for addr, t in ins:
+            m = re.search(r"\bBRA\b.*?0x([0-9a-f]+)", t)
+            if m and int(m.group(1), 16) < addr:
+                loops.append((int(m.group(1), 16), addr))
+        inner = [l for l in loops if not any(o != l and o[0] >= l[0] and o[1] <= l[1] for o in loops)]
+        lo, hi = max(inner, key=lambda l: l[1] - l[0])      # the step loop is the longest innermost loop
+        c = collections.Counter()
+        for addr, t in ins:
+            if lo <= addr <= hi:
+                c[re.sub(r"^@!?U?P\d+\s+", "", t).split()[0].split(".")[0]] += 1
+        fp = c["DFMA"] + c["DMUL"] + c["DADD"]
+        mix = {"dfma": c["DFMA"], "dmul": c["DMUL"], "dadd": c["DADD"], "other": sum(c.values()) - fp,
+               "flops": 2 * c["DFMA"] + c["DMUL"] + c["DADD"]}
+        _cache[key] = mix
+        return mix
+    raise KeyError(tag)
+
+
+if __name__ == "__main__":
+    for order in (4, 6):
+        for tangent in (False, True):
+            for level in range(5):
+                print(order, tangent, level, integrate_step_mix(order, tangent, level))

@@ -81,7 +81,7 @@ def test_validation_happens_on_the_host(aw):
     buf = (C.c_double * 1024)()
     base = C.addressof(buf)
     base += (-base) % 16
-    st = AwState(64, 64, base, None, base, None, base, 1.0, 1e-2, 0.0, 0, 4, 1, None)
+    st = AwState(64, 64, base, None, base, None, base, 1.0, 1e-2, 0.0, 0, 4, 1, 0, 0, None)
     g = Grid(8, 8, -1.0, 1.0, -1.0, 1.0, 0, 0, 0.0, 0.0, 0.0, 1, 0)
     EINVAL, ERANGE, ESTATE = -1, -3, -4
     assert L.aw_integrate(C.byref(st), 63, 100, 0.01, 100) == EINVAL        # n mismatch
@@ -103,6 +103,15 @@ def test_validation_happens_on_the_host(aw):
     st.q = base + 8                                                        # misaligned plane
     assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == EINVAL
     st.q = base
+    # trigonometry level picked on the host from the largest drift angle (include/aw.h, aw_integrate)
+    lv = lambda dt: L.aw_trig_level(C.byref(st), dt)
+    assert [lv(0.005), lv(-0.005), lv(0.01), lv(0.015), lv(0.03), lv(0.05), lv(0.5)] == [1, 1, 2, 3, 4, 0, 0]
+    st.order = 6                                      # largest |c_s| is 0.7845 instead of 1.3512
+    assert [lv(0.005), lv(0.01), lv(0.02), lv(0.05), lv(0.07)] == [1, 2, 3, 4, 0]
+    st.order, st.trig = 4, 1
+    assert lv(0.005) == 0
+    st.trig = 0
+    assert lv(0.0) == EINVAL
     # init_shell
     assert L.aw_init_shell(C.byref(st), C.byref(g), 1.0, 0.6, 0) == ERANGE  # E - 2|eps| <= 0
     g.gx = 7
@@ -121,7 +130,7 @@ def test_validation_happens_on_the_host(aw):
     assert L.aw_density(C.byref(st), None, 16, 16, -1.0, 1.0, 0, None) == EINVAL
     assert L.aw_density(C.byref(st), base, 0, 16, -1.0, 1.0, 0, None) == EINVAL
     # zero-size ensemble: every call is a no-op that never reaches the device
-    z = AwState(0, 0, None, None, None, None, None, 1.0, 1e-2, 0.0, 0, 4, 1, None)
+    z = AwState(0, 0, None, None, None, None, None, 1.0, 1e-2, 0.0, 0, 4, 1, 0, 0, None)
     g0 = Grid(0, 0, -1.0, 1.0, -1.0, 1.0, 0, 0, 0.0, 0.0, 0.0, 1, 0)
     assert L.aw_integrate(C.byref(z), 0, 100, 0.01, 100) == 0
     assert L.aw_init_shell(C.byref(z), C.byref(g0), 1.0, 1e-2, 0) == EINVAL  # gx <= 0
