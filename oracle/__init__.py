@@ -67,15 +67,22 @@ def lib():
         L.awo_uniform.argtypes = [C.c_uint64] * 3
         L.awo_common_tangent.argtypes = [C.c_uint64, _dp]
         L.awo_steps.argtypes = [_dp, _dp, C.c_int, C.c_double, C.c_double, C.c_int64]
-        L.awo_checkpoint.argtypes = [_dp, _dp, _dp, _i32p, C.c_double]
+        L.awo_checkpoint.argtypes = [_dp, _dp, _dp, _i32p, C.c_double, _dp]
         L.awo_init_shell.argtypes = [C.POINTER(Grid), C.c_double, C.c_double, C.c_uint64, C.c_int64,
                                      C.c_int64, _dp, _dp, _dp, _i32p, _u8p]
         L.awo_integrate.argtypes = [C.c_int64, C.c_int64, _dp, _dp, _dp, _i32p, _u8p, C.c_double,
-                                    C.c_int, C.c_int64, C.c_double, C.c_int64, C.c_int64, C.c_int64]
+                                    C.c_int, C.c_int64, C.c_double, C.c_int64, C.c_int64, C.c_int64, _dp]
         L.awo_indicator.argtypes = [C.c_int64, C.c_int64, _dp, _u8p, C.c_double, C.c_int, C.c_double,
                                     _dp, _u8p]
         L.awo_density.argtypes = [C.c_int64, C.c_int64, _dp, _u8p, _u32p, C.c_int32, C.c_int32,
                                   C.c_double, C.c_double, _u64p]
+        L.awo_mark.argtypes = [C.c_int64, _dp, _i32p, _dp, _i32p]
+        L.awo_velocity.argtypes = [C.c_int64, C.c_int64, _dp, _i32p, _dp, _i32p, _u8p, C.c_double, C.c_double,
+                                   C.c_int, _dp]
+        L.awo_density_velocity.argtypes = [C.c_int64, C.c_int64, _dp, _i32p, _dp, _i32p, _u8p, C.c_double,
+                                           C.c_double, C.c_int, _u32p, C.c_int32, C.c_int32, C.c_double,
+                                           C.c_double, _u64p]
+        L.awo_delta_p.argtypes = [C.c_int64, C.c_int64, _dp, _dp, _u8p, _dp]
         _lib = L
     return _lib
 
@@ -142,12 +149,13 @@ def steps(q, tw, order, dt, eps, nsteps):
     return q, tw
 
 
-def checkpoint(q, tw, acc, wind, eps):
+def checkpoint(q, tw, acc, wind, eps, surv=None):
     q = np.array(q, dtype=np.float64)
     tw = None if tw is None else np.array(tw, dtype=np.float64)
     acc = np.array(acc, dtype=np.float64)
     wind = None if wind is None else np.array(wind, dtype=np.int32)
-    st = lib().awo_checkpoint(_p(q, _dp), _p(tw, _dp), _p(acc, _dp), _p(wind, _i32p), eps)
+    surv = None if surv is None else np.array(surv, dtype=np.float64)
+    st = lib().awo_checkpoint(_p(q, _dp), _p(tw, _dp), _p(acc, _dp), _p(wind, _i32p), eps, _p(surv, _dp))
     return q, tw, acc, wind, st
 
 
@@ -169,6 +177,10 @@ class State:
         self.t = 0.0
         self.step = 0
         self.order = 4
+        self.qref = None        # snapshot taken by mark(): start of the averaging window
+        self.windref = None
+        self.tref = 0.0
+        self.surv = None        # survivor rectangle (lo_x, hi_x, lo_y, hi_y) or None
 
     def copy(self):
         s = State(self.n, self.w is not None, self.wind is not None, self.pitch)
@@ -180,6 +192,9 @@ class State:
             s.wind[:] = self.wind
         s.status[:] = self.status
         s.E, s.eps, s.t, s.step, s.order = self.E, self.eps, self.t, self.step, self.order
+        s.qref = None if self.qref is None else self.qref.copy()
+        s.windref = None if self.windref is None else self.windref.copy()
+        s.tref, s.surv = self.tref, self.surv
         return s
 
 
@@ -196,9 +211,10 @@ def integrate(state, steps, dt, stride, k0=0, k1=None, advance_clock=True):
     """Integrate trajectories [k0, k1) (default all).  Single-threaded; callers may run disjoint
     ranges from several Python threads (ctypes drops the GIL) — the arithmetic is per trajectory."""
     k1 = state.n if k1 is None else k1
+    surv = None if state.surv is None else np.array(state.surv, dtype=np.float64)
     rc = lib().awo_integrate(state.n, state.pitch, _p(state.q, _dp), _p(state.w, _dp),
                              _p(state.acc, _dp), _p(state.wind, _i32p), _p(state.status, _u8p),
-                             state.eps, state.order, steps, dt, stride, k0, k1)
+                             state.eps, state.order, steps, dt, stride, k0, k1, _p(surv, _dp))
     assert rc == 0, rc
     if advance_clock:
         state.t += steps * abs(dt)
@@ -227,3 +243,46 @@ def density(state, hist, lo, hi, dropped=None):
                            _p(hist, _u32p), gx, gy, lo, hi, _p(d, _u64p))
     assert rc == 0, rc
     return d
+
+
+def mark(state):
+    """Snapshot (q, wind) as the start of an averaging window / the reference P(0) of P:37."""
+    state.qref = np.zeros_like(state.q)
+    state.windref = None if state.wind is None else np.zeros_like(state.wind)
+    rc = lib().awo_mark(state.pitch, _p(state.q, _dp), _p(state.wind, _i32p), _p(state.qref, _dp),
+                        _p(state.windref, _i32p))
+    assert rc == 0, rc
+    state.tref = state.t
+    return state
+
+
+def velocity(state, projected=True):
+    """[3, n] averaged finite-time velocity over [tref, t], centrally projected on S if asked."""
+    out = np.zeros((3, state.n))
+    rc = lib().awo_velocity(state.n, state.pitch, _p(state.q, _dp), _p(state.wind, _i32p),
+                            _p(state.qref, _dp), _p(state.windref, _i32p), _p(state.status, _u8p),
+                            state.E, state.t - state.tref, 1 if projected else 0, _p(out, _dp))
+    assert rc == 0, rc
+    return out
+
+
+def density_velocity(state, hist, lo, hi, hemi=1, dropped=None):
+    """Add the projected averaged velocities (Vhat_x, Vhat_y) of one hemisphere (1: z >= 0, 2: z < 0,
+    3: both) into hist[gy, gx]; returns dropped."""
+    gy, gx = hist.shape
+    d = np.zeros(1, dtype=np.uint64) if dropped is None else dropped
+    rc = lib().awo_density_velocity(state.n, state.pitch, _p(state.q, _dp), _p(state.wind, _i32p),
+                                    _p(state.qref, _dp), _p(state.windref, _i32p), _p(state.status, _u8p),
+                                    state.E, state.t - state.tref, hemi, _p(hist, _u32p), gx, gy, lo, hi,
+                                    _p(d, _u64p))
+    assert rc == 0, rc
+    return d
+
+
+def delta_p(state):
+    """||P(t) - P(tref)|| per trajectory."""
+    out = np.zeros(state.n)
+    rc = lib().awo_delta_p(state.n, state.pitch, _p(state.q, _dp), _p(state.qref, _dp),
+                           _p(state.status, _u8p), _p(out, _dp))
+    assert rc == 0, rc
+    return out

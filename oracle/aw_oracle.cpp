@@ -22,7 +22,9 @@
 // Pins (tests/test_oracle_pins.py, run with -m "not gpu"): eps=0 closed form, energy-error order
 // 4 / 6, order conditions of the weights, reversibility, symplectic 6x6 tangent map, tangent
 // vs finite differences, pendulum reduction vs the complete elliptic integral, invariant subspaces
-// (P:79), shell layer, IC energy, histogram brute force.  No function here is
+// (P:79), shell layer, IC energy, histogram brute force; averaged velocity vs eps=0 closed
+// form, vs an unwrapped brute-force run and vs the pendulum rotation frequency 2 pi / T(h); central
+// projection on a hand case; survivor filter vs a stepwise brute force.  No function here is
 // "parity unpinned" except where DESIGN.md §3 says so (the paper's figures and its dE<1e-8 remark).
 
 #include <cmath>
@@ -174,8 +176,12 @@ const double INV_2PI = 0.15915494309189535;      // double nearest 1/(2 pi)
 const double TWO_PI_HI = 6.283185307179586;      // double nearest 2 pi  (0x1.921fb54442d18p+2)
 const double TWO_PI_LO = 2.4492935982947064e-16; // 2 pi - TWO_PI_HI
 
-// acc = {logsum, fli_max, H0, dH_max}; wind may be nullptr; returns the new status
-inline int checkpoint(double q[6], double *tw, double acc[4], int32_t *wind, double eps) {
+// acc = {logsum, fli_max, H0, dH_max}; wind may be nullptr; returns the new status.
+// surv (may be nullptr) = {lo_x, hi_x, lo_y, hi_y}: the survivor filter of P:99 ("tracked only those
+// trajectories which remained within the area during the whole observation time"; R25): a trajectory
+// whose (px, py) is outside the half-open rectangle at a checkpoint gets status 3 and is frozen there.
+inline int checkpoint(double q[6], double *tw, double acc[4], int32_t *wind, double eps,
+                      const double *surv = nullptr) {
   // (i) renormalise the tangent vector and accumulate the log of its growth
   if (tw) {
     double s2 = tw[0] * tw[0];
@@ -202,7 +208,9 @@ inline int checkpoint(double q[6], double *tw, double acc[4], int32_t *wind, dou
   for (int i = 0; i < 6; ++i) finite = finite && std::isfinite(q[i]);
   if (tw)
     for (int i = 0; i < 6; ++i) finite = finite && std::isfinite(tw[i]);
-  return finite ? 1 : 2;
+  if (!finite) return 2;
+  if (surv && !(q[3] >= surv[0] && q[3] < surv[1] && q[4] >= surv[2] && q[4] < surv[3])) return 3;
+  return 1;
 }
 
 // ---------------------------------------------------------------- counter-based randomness (R11)
@@ -247,7 +255,8 @@ struct awo_grid {
   int32_t gx, gy;
   double lo_x, hi_x, lo_y, hi_y;
   int32_t angle_mode;    // 0: all angles 0; 1: U[0,2pi) from seed
-  int32_t shape;         // 0: grid; 1: uniform disk (cx,cy,r); 2: Gaussian (cx,cy,sigma=r)
+  int32_t shape;         // 0: grid; 1: uniform disk (cx,cy,r); 2: Gaussian (cx,cy,sigma=r);
+                         // 3: uniform on the whole sphere S (R28)
   double cx, cy, r;
   int32_t pz_sign;       // +1 or -1
   int32_t tangent_mode;  // 0: one common seeded unit vector; 1: per trajectory
@@ -275,8 +284,8 @@ int awo_steps(double *q, double *tw, int order, double dt, double eps, int64_t n
 }
 
 // One checkpoint on ONE trajectory (exposed so tests can exercise the wrap and renormalisation alone).
-int awo_checkpoint(double *q, double *tw, double *acc, int32_t *wind, double eps) {
-  return checkpoint(q, tw, acc, wind, eps);
+int awo_checkpoint(double *q, double *tw, double *acc, int32_t *wind, double eps, const double *surv) {
+  return checkpoint(q, tw, acc, wind, eps, surv);
 }
 
 // a1: initial conditions on the energy shell (R6, R8-R12, R17, R18).
@@ -289,34 +298,50 @@ int awo_init_shell(const awo_grid *g, double E, double eps, uint64_t seed, int64
   const double nan = std::numeric_limits<double>::quiet_NaN();
   for (int64_t k = 0; k < n; ++k) {
     const int64_t i = k % g->gx, j = k / g->gx;
-    double px, py;
-    if (g->shape == 0) {
-      px = g->lo_x + ((double)i + 0.5) * (g->hi_x - g->lo_x) / (double)g->gx;
-      py = g->lo_y + ((double)j + 0.5) * (g->hi_y - g->lo_y) / (double)g->gy;
-    } else {
-      const double u1 = uniform01(seed, (uint64_t)k, 3), u2 = uniform01(seed, (uint64_t)k, 4);
-      const double ang = TWO_PI_HI * u2;
-      const double rad = (g->shape == 1) ? g->r * std::sqrt(u1)
-                                         : g->r * std::sqrt(-2.0 * std::log(1.0 - u1));
-      px = g->cx + rad * std::cos(ang);
-      py = g->cy + rad * std::sin(ang);
-    }
     double X[3] = {0.0, 0.0, 0.0};
     if (g->angle_mode == 1)
       for (int al = 0; al < 3; ++al) X[al] = TWO_PI_HI * uniform01(seed, (uint64_t)k, (uint64_t)al);
-    // third action from the energy condition H = E
-    double R = 2.0 * (E - eps * Hp(X[0], X[1], X[2]));
-    R = R - px * px;
-    R = R - py * py;
     double st[6];
-    if (R < 0.0 || !(R == R)) {
-      status[k] = 0;
-      for (int c = 0; c < 6; ++c) st[c] = nan;
-    } else {
+    if (g->shape == 3) {
+      // P:85 "initial conditions uniformly distributed over the sphere S": direction uniform on the unit
+      // sphere (cos(theta) = 1 - 2 u3 uniform in (-1, 1], phi = 2 pi u4), |P| from the energy condition
+      // H = E: |P|^2 = 2 (E - eps H_p(X)) > 0 always (E > 2|eps|), so no point is off the shell (R28).
+      const double u1 = uniform01(seed, (uint64_t)k, 3), u2 = uniform01(seed, (uint64_t)k, 4);
+      const double ct = 1.0 - 2.0 * u1;
+      const double sth = std::sqrt((1.0 - ct) * (1.0 + ct));
+      const double ang = TWO_PI_HI * u2;
+      const double pn = std::sqrt(2.0 * (E - eps * Hp(X[0], X[1], X[2])));
       status[k] = 1;
       st[0] = X[0]; st[1] = X[1]; st[2] = X[2];
-      st[3] = px; st[4] = py;
-      st[5] = (g->pz_sign < 0 ? -1.0 : 1.0) * std::sqrt(R);
+      st[3] = pn * (sth * std::cos(ang));
+      st[4] = pn * (sth * std::sin(ang));
+      st[5] = (g->pz_sign < 0 ? -1.0 : 1.0) * (pn * ct);
+    } else {
+      double px, py;
+      if (g->shape == 0) {
+        px = g->lo_x + ((double)i + 0.5) * (g->hi_x - g->lo_x) / (double)g->gx;
+        py = g->lo_y + ((double)j + 0.5) * (g->hi_y - g->lo_y) / (double)g->gy;
+      } else {
+        const double u1 = uniform01(seed, (uint64_t)k, 3), u2 = uniform01(seed, (uint64_t)k, 4);
+        const double ang = TWO_PI_HI * u2;
+        const double rad = (g->shape == 1) ? g->r * std::sqrt(u1)
+                                           : g->r * std::sqrt(-2.0 * std::log(1.0 - u1));
+        px = g->cx + rad * std::cos(ang);
+        py = g->cy + rad * std::sin(ang);
+      }
+      // third action from the energy condition H = E
+      double R = 2.0 * (E - eps * Hp(X[0], X[1], X[2]));
+      R = R - px * px;
+      R = R - py * py;
+      if (R < 0.0 || !(R == R)) {
+        status[k] = 0;
+        for (int c = 0; c < 6; ++c) st[c] = nan;
+      } else {
+        status[k] = 1;
+        st[0] = X[0]; st[1] = X[1]; st[2] = X[2];
+        st[3] = px; st[4] = py;
+        st[5] = (g->pz_sign < 0 ? -1.0 : 1.0) * std::sqrt(R);
+      }
     }
     for (int c = 0; c < 6; ++c) q[c * pitch + k] = st[c];
     acc[0 * pitch + k] = 0.0;                                          // logsum
@@ -336,9 +361,10 @@ int awo_init_shell(const awo_grid *g, double E, double eps, uint64_t seed, int64
 }
 
 // a2 + a3 + a4: integrate trajectories k in [k0, k1) for `steps` steps, checkpoint every `stride`.
+// surv = NULL or the survivor rectangle {lo_x, hi_x, lo_y, hi_y} (R25).
 int awo_integrate(int64_t n, int64_t pitch, double *q, double *w, double *acc, int32_t *wind,
                   uint8_t *status, double eps, int order, int64_t steps, double dt, int64_t stride,
-                  int64_t k0, int64_t k1) {
+                  int64_t k0, int64_t k1, const double *surv) {
   if (!q || !acc || !status || stride <= 0 || steps < 0 || steps % stride != 0) return -1;
   if (k0 < 0 || k1 > n || pitch < n) return -1;
   double a[10], b[9];
@@ -355,7 +381,7 @@ int awo_integrate(int64_t n, int64_t pitch, double *q, double *w, double *acc, i
     int stt = 1;
     for (int64_t c0 = 0; c0 < steps; c0 += stride) {
       for (int64_t i = 0; i < stride; ++i) one_step(s, w ? t : nullptr, S, a, b);
-      stt = checkpoint(s, w ? t : nullptr, ac, wd, eps);
+      stt = checkpoint(s, w ? t : nullptr, ac, wd, eps, surv);
       if (stt != 1) break;
     }
     status[k] = (uint8_t)stt;
@@ -395,6 +421,102 @@ int awo_density(int64_t n, int64_t pitch, const double *q, const uint8_t *status
     if (ax >= 0.0 && ax < (double)gx && ay >= 0.0 && ay < (double)gy)
       hist[(int64_t)ay * gx + (int64_t)ax] += 1u;
     else if (dropped) *dropped += 1ull;
+  }
+  return 0;
+}
+
+// ---------------------------------------------------------------- the paper's own indicator
+//
+// "For every trajectory from the ensemble we calculate the vector of the averaged finite-time velocity
+//  V^i(t) with the components V_a(t) = [X_a(t + Dt) - X_a(t)] / Dt", where X is the unwrapped
+// coordinate: the checkpoint wraps the angles and counts whole turns (R7), so
+//   X_a(t + Dt) - X_a(t) = (x_a - xref_a) + 2 pi (wind_a - windref_a)                        (R27)
+// with (xref, windref) the snapshot taken at time t (awo_mark).  "Finally we use the central projection
+// of the point V on the surface of the sphere" S: P^2 = 2E (P:171 fn. 26): Vhat = sqrt(2E) V / |V|.
+// Every product, sum, quotient and root below is rounded separately, in exactly this order.
+
+// snapshot of the state at the start of an averaging window: qref <- q (6 planes), windref <- wind
+int awo_mark(int64_t pitch, const double *q, const int32_t *wind, double *qref, int32_t *windref) {
+  if (!q || !qref) return -1;
+  std::memcpy(qref, q, sizeof(double) * 6 * (size_t)pitch);
+  if (wind && windref) std::memcpy(windref, wind, sizeof(int32_t) * 3 * (size_t)pitch);
+  return 0;
+}
+
+namespace {
+// V (averaged velocity) and Vhat (its central projection on S) of trajectory k; false if |V| is zero
+// or not finite (nothing to project).
+inline bool averaged_velocity(int64_t k, int64_t pitch, const double *q, const int32_t *wind,
+                              const double *qref, const int32_t *windref, double E, double Dt,
+                              double V[3], double Vhat[3]) {
+  for (int a = 0; a < 3; ++a) {
+    const double dxw = q[a * pitch + k] - qref[a * pitch + k];
+    const int32_t dk = (wind && windref) ? wind[a * pitch + k] - windref[a * pitch + k] : 0;
+    const double dX = (double)dk * TWO_PI_HI + dxw;
+    V[a] = dX / Dt;
+  }
+  double n2 = V[0] * V[0];
+  n2 = n2 + V[1] * V[1];
+  n2 = n2 + V[2] * V[2];
+  const double nrm = std::sqrt(n2);
+  if (!(nrm > 0.0) || !std::isfinite(nrm)) return false;
+  const double scale = std::sqrt(2.0 * E) / nrm;
+  for (int a = 0; a < 3; ++a) Vhat[a] = V[a] * scale;
+  return true;
+}
+}  // namespace
+
+// out[3*n] (planes of n): kind 0 -> V, kind 1 -> Vhat; NaN where the trajectory is not live or |V| = 0
+int awo_velocity(int64_t n, int64_t pitch, const double *q, const int32_t *wind, const double *qref,
+                 const int32_t *windref, const uint8_t *status, double E, double Dt, int kind, double *out) {
+  if (!q || !qref || !status || !out || !(Dt > 0.0)) return -1;
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+  for (int64_t k = 0; k < n; ++k) {
+    double V[3], Vh[3];
+    const bool ok = status[k] == 1 && averaged_velocity(k, pitch, q, wind, qref, windref, E, Dt, V, Vh);
+    for (int a = 0; a < 3; ++a) out[a * n + k] = ok ? (kind == 0 ? V[a] : Vh[a]) : nan;
+  }
+  return 0;
+}
+
+// Density F_Dt(V; t) of the projected averaged velocity on the sphere S, as the sphere seen along
+// the third axis (R26): bins over (Vhat_x, Vhat_y) exactly as awo_density bins (px, py); hemi = 1 counts
+// the hemisphere Vhat_z >= 0, hemi = 2 the hemisphere Vhat_z < 0, hemi = 3 both (folded).  Points of
+// the other hemisphere, outside [lo, hi)^2, or with |V| = 0 go to *dropped.  Adds into hist.
+int awo_density_velocity(int64_t n, int64_t pitch, const double *q, const int32_t *wind, const double *qref,
+                         const int32_t *windref, const uint8_t *status, double E, double Dt, int hemi,
+                         uint32_t *hist, int32_t gx, int32_t gy, double lo, double hi, uint64_t *dropped) {
+  if (!(hi > lo) || gx <= 0 || gy <= 0 || !(Dt > 0.0) || hemi < 1 || hemi > 3) return -1;
+  const double fx = (double)gx / (hi - lo), fy = (double)gy / (hi - lo);
+  for (int64_t k = 0; k < n; ++k) {
+    if (status[k] != 1) continue;
+    double V[3], Vh[3];
+    bool in = averaged_velocity(k, pitch, q, wind, qref, windref, E, Dt, V, Vh);
+    if (in) in = (hemi == 3) || (hemi == 1 ? Vh[2] >= 0.0 : Vh[2] < 0.0);
+    if (in) {
+      const double ax = std::floor((Vh[0] - lo) * fx), ay = std::floor((Vh[1] - lo) * fy);
+      in = ax >= 0.0 && ax < (double)gx && ay >= 0.0 && ay < (double)gy;
+      if (in) hist[(int64_t)ay * gx + (int64_t)ax] += 1u;
+    }
+    if (!in && dropped) *dropped += 1ull;
+  }
+  return 0;
+}
+
+// Drift detector of P:37: dP(t) = ||P(t) - P(0)||, with P(0) the marked snapshot.  out[n], NaN if not live.
+int awo_delta_p(int64_t n, int64_t pitch, const double *q, const double *qref, const uint8_t *status,
+                double *out) {
+  if (!q || !qref || !status || !out) return -1;
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+  for (int64_t k = 0; k < n; ++k) {
+    if (status[k] != 1) { out[k] = nan; continue; }
+    const double d0 = q[3 * pitch + k] - qref[3 * pitch + k];
+    const double d1 = q[4 * pitch + k] - qref[4 * pitch + k];
+    const double d2 = q[5 * pitch + k] - qref[5 * pitch + k];
+    double s2 = d0 * d0;
+    s2 = s2 + d1 * d1;
+    s2 = s2 + d2 * d2;
+    out[k] = std::sqrt(s2);
   }
   return 0;
 }
