@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define AW_VERSION 100 /* 1.0.0 */
+#define AW_VERSION 110 /* 1.1.0 */
 
 #if defined(__GNUC__)
 #define AW_API __attribute__((visibility("default")))
@@ -51,12 +51,15 @@ typedef enum {
   AW_ESTATE = -4  /* aw_state not usable for this call (not initialised, no tangent planes ...) */
 } aw_status;
 
-/* indicator kinds for aw_indicator (R13, R14) */
-enum { AW_IND_FLI = 0, AW_IND_FTLE = 1, AW_IND_DH = 2, AW_IND_CLASS = 3 };
+/* indicator kinds for aw_indicator (R13, R14; DP: P:37; VX..VZ: P:67 + fn. 26) */
+enum { AW_IND_FLI = 0, AW_IND_FTLE = 1, AW_IND_DH = 2, AW_IND_CLASS = 3,
+       AW_IND_DP = 4, AW_IND_VX = 5, AW_IND_VY = 6, AW_IND_VZ = 7 };
+/* aw_density modes: instantaneous actions (BASELINE) or the paper's projected averaged velocity (R19, R26) */
+enum { AW_DENS_ACTION = 0, AW_DENS_VEL_UPPER = 1, AW_DENS_VEL_LOWER = 2, AW_DENS_VEL_BOTH = 3 };
 /* aw_grid.shape */
-enum { AW_SHAPE_GRID = 0, AW_SHAPE_DISK = 1, AW_SHAPE_GAUSS = 2 };
+enum { AW_SHAPE_GRID = 0, AW_SHAPE_DISK = 1, AW_SHAPE_GAUSS = 2, AW_SHAPE_SPHERE = 3 };
 /* per-trajectory status byte */
-enum { AW_ST_OFFSHELL = 0, AW_ST_LIVE = 1, AW_ST_NONFINITE = 2 };
+enum { AW_ST_OFFSHELL = 0, AW_ST_LIVE = 1, AW_ST_NONFINITE = 2, AW_ST_LEFT = 3 };
 
 /* Static, never-freed description of a status code. */
 AW_API const char *aw_strerror(int code);
@@ -85,8 +88,15 @@ typedef struct {
   int32_t ready;   /* set to 1 by aw_init_shell (or by the caller after uploading a state)    */
   int32_t trig;    /* 0 (default): running (sin, cos) pairs advanced by rotations, see aw_integrate;
                       1: evaluate the device sincos at every stage                            */
-  int32_t reserved; /* must be 0                                                              */
+  int32_t survive; /* 1: survivor filter on (R25), see surv_* below; 0 (default): off    */
   void *stream;    /* cudaStream_t; NULL = legacy default stream                              */
+  double *qref;    /* device, 6*pitch: snapshot of q written by aw_mark (start of the averaging
+                      window of P:67 / the P(0) of P:37); NULL = no snapshot planes             */
+  int32_t *windref; /* device, 3*pitch: snapshot of wind; NULL iff wind is NULL                */
+  double tref;     /* model time of the snapshot (set by aw_mark)                             */
+  double surv_lo_x, surv_hi_x, surv_lo_y, surv_hi_y; /* launch rectangle of the survivor filter:
+                      a trajectory whose (px, py) is outside [lo_x, hi_x) x [lo_y, hi_y) at a
+                      checkpoint gets status AW_ST_LEFT and is frozen there                    */
 } aw_state;
 
 /* Initial-condition family (P:85 whole region, P:87 patch, P:97 cloud; R6, R8, R9, R12, R17, R18). */
@@ -96,7 +106,11 @@ typedef struct {
                                     px = lo_x + (i + 1/2)(hi_x - lo_x)/gx, py likewise with j  */
   int32_t angle_mode;           /* 0: all angles 0;  1: angle_a = 2pi * u(seed, k, a), a=0,1,2 */
   int32_t shape;                /* AW_SHAPE_*: DISK  (px,py) = (cx,cy) + r sqrt(u3) (cos,sin)(2pi u4)
-                                               GAUSS (px,py) = (cx,cy) + r sqrt(-2 ln(1-u3)) (cos,sin)(2pi u4) */
+                                               GAUSS (px,py) = (cx,cy) + r sqrt(-2 ln(1-u3)) (cos,sin)(2pi u4)
+                                               SPHERE (R28) direction uniform on the unit sphere:
+                                                 cos(th) = 1 - 2 u3, phi = 2pi u4, |P| = sqrt(2(E - eps H_p(X)))
+                                                 P = |P| (sin th cos phi, sin th sin phi, pz_sign cos th);
+                                                 never off the shell; lo/hi/cx/cy/r unused        */
   double cx, cy, r;
   int32_t pz_sign;              /* +1 (default, upper hemisphere; R9) or -1                    */
   int32_t tangent_mode;         /* 0: one common seeded unit vector (R12); 1: per trajectory   */
@@ -127,7 +141,10 @@ AW_API int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps,
  * tangent vector goes through the exact derivative of the same map (R3).  Every `stride` steps the
  * fused checkpoint runs (R4): renormalise the tangent vector, logsum += ln|w|, fli = max(fli, logsum);
  * dH_max = max(dH_max, |H - H0|); wrap the angles to [-pi,pi] counting whole turns into wind (R7);
- * a non-finite state sets status 2 and freezes the trajectory.
+ * a non-finite state sets status 2 and freezes the trajectory; with s->survive == 1 a trajectory whose
+ * (px, py) is outside the launch rectangle s->surv_* at a checkpoint gets status 3 (AW_ST_LEFT) and is
+ * frozen at that checkpoint ("tracked only those trajectories which remained within the area during
+ * the whole observation time"; R25) — it is then skipped by every later call, image and histogram.
  * n must equal s->n.  steps >= 0, stride > 0, steps % stride == 0; dt != 0 finite (dt < 0 integrates
  * backwards).  steps == 0 or n == 0 is a no-op.  AW_ERANGE if stride*|dt|*sqrt(2(E+2|eps|)) >= 1024
  * (the angle would leave the range the two-constant argument reduction handles exactly, R7).
@@ -144,17 +161,36 @@ AW_API int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps,
 #define AW_MAX_STEPS_PER_LAUNCH 20000
 AW_API int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t stride);
 
+/* §8(f) 1-2 — snapshot of the state: qref <- q, windref <- wind, tref <- t (device-to-device copies on
+ * s->stream).  It is the X(t) of the averaging window [t, t + Dt] of P:67 and the P(0) of the drift
+ * detector dP(t) = |P(t) - P(0)| of P:37.  AW_ESTATE if s->qref == NULL, if wind and windref are not
+ * both NULL or both non-NULL, or if the state is not ready. */
+AW_API int aw_mark(aw_state *s);
+
 /* §8(a) a5 — indicator image.  kind AW_IND_FLI: fli_max; AW_IND_FTLE: logsum / s->t; AW_IND_DH:
  * dH_max -> out_dev = n doubles (device), NaN where status != 1.  AW_IND_CLASS: out_dev = n bytes
  * (device), 1 if fli_max > thr else 0, 255 where status != 1 (R14; pass thr = log(t) + 3 for the
  * default).  AW_ESTATE if a tangent indicator is asked of a state without tangent planes, or FTLE
- * at t == 0. */
+ * at t == 0.
+ * §8(f): AW_IND_DP: |P - Pref| (three rounded squares summed left to right, IEEE sqrt).
+ * AW_IND_VX / VY / VZ: component of the projected averaged velocity Vhat (see aw_density), NaN where
+ * the trajectory is not live or |V| = 0.  These need s->qref (AW_ESTATE if NULL); VX..VZ also need
+ * s->t > s->tref. */
 AW_API int aw_indicator(const aw_state *s, int kind, double thr, void *out_dev);
 
 /* §8(a) a6 — visited-cell density over the first two actions (R19, R20).  For each live
  * trajectory ix = floor((px - lo) * (gx/(hi - lo))), iy likewise with gy; inside -> hist[iy*gx + ix]
  * += 1, else *dropped_dev += 1 (dropped_dev may be NULL).  ADDS into hist_dev (device, gx*gy uint32;
- * the caller zeroes it) so repeated calls give the time-accumulated density.  mode must be 0. */
+ * the caller zeroes it) so repeated calls give the time-accumulated density.
+ * mode AW_DENS_ACTION (0): the point binned is the instantaneous (px, py) (BASELINE configs[4]).
+ * modes 1-3, §8(f) 1 — the paper's own indicator (P:67, P:171 fn. 26; R26, R27): the point binned is
+ * (Vhat_x, Vhat_y) of the averaged finite-time velocity over the window [tref, t] since aw_mark,
+ *   dX_a = (double)(wind_a - windref_a) * 2pi_hi + (x_a - xref_a),   V_a = dX_a / (t - tref),
+ *   |V| = sqrt((Vx Vx + Vy Vy) + Vz Vz),   Vhat_a = V_a * (sqrt(2E) / |V|)     (central projection on S),
+ * every operation rounded separately in this order (no FMA), i.e. the sphere S seen along the third
+ * axis: AW_DENS_VEL_UPPER counts the hemisphere Vhat_z >= 0, _LOWER Vhat_z < 0, _BOTH both (folded);
+ * the other hemisphere, |V| = 0 or non-finite, and points outside [lo, hi)^2 go to *dropped_dev.
+ * AW_ESTATE if s->qref == NULL or !(s->t > s->tref). */
 AW_API int aw_density(const aw_state *s, uint32_t *hist_dev, int32_t gx, int32_t gy, double lo, double hi,
                int mode, uint64_t *dropped_dev);
 

@@ -14,6 +14,10 @@ _LIBPATH = os.path.join(_HERE, "libaw.so")
 
 AW_OK, AW_EINVAL, AW_ECUDA, AW_ERANGE, AW_ESTATE = 0, -1, -2, -3, -4
 AW_IND_FLI, AW_IND_FTLE, AW_IND_DH, AW_IND_CLASS = 0, 1, 2, 3
+AW_IND_DP, AW_IND_VX, AW_IND_VY, AW_IND_VZ = 4, 5, 6, 7
+AW_DENS_ACTION, AW_DENS_VEL_UPPER, AW_DENS_VEL_LOWER, AW_DENS_VEL_BOTH = 0, 1, 2, 3
+AW_SHAPE_GRID, AW_SHAPE_DISK, AW_SHAPE_GAUSS, AW_SHAPE_SPHERE = 0, 1, 2, 3
+AW_ST_OFFSHELL, AW_ST_LIVE, AW_ST_NONFINITE, AW_ST_LEFT = 0, 1, 2, 3
 
 
 class AwError(RuntimeError):
@@ -30,8 +34,11 @@ class AwState(C.Structure):
                 ("q", C.c_void_p), ("w", C.c_void_p), ("acc", C.c_void_p), ("wind", C.c_void_p),
                 ("status", C.c_void_p),
                 ("E", C.c_double), ("eps", C.c_double), ("t", C.c_double), ("step", C.c_int64),
-                ("order", C.c_int32), ("ready", C.c_int32), ("trig", C.c_int32), ("reserved", C.c_int32),
-                ("stream", C.c_void_p)]
+                ("order", C.c_int32), ("ready", C.c_int32), ("trig", C.c_int32), ("survive", C.c_int32),
+                ("stream", C.c_void_p),
+                ("qref", C.c_void_p), ("windref", C.c_void_p), ("tref", C.c_double),
+                ("surv_lo_x", C.c_double), ("surv_hi_x", C.c_double),
+                ("surv_lo_y", C.c_double), ("surv_hi_y", C.c_double)]
 
 
 class Grid(C.Structure):
@@ -79,6 +86,7 @@ def lib():
         L.aw_state_bytes.argtypes = [i64, C.c_int, C.c_int, C.POINTER(i64)]
         L.aw_init_shell.argtypes = [C.POINTER(AwState), C.POINTER(Grid), dbl, dbl, u64]
         L.aw_integrate.argtypes = [C.POINTER(AwState), i64, i64, dbl, i64]
+        L.aw_mark.argtypes = [C.POINTER(AwState)]
         L.aw_indicator.argtypes = [C.POINTER(AwState), C.c_int, dbl, vp]
         L.aw_density.argtypes = [C.POINTER(AwState), vp, i32, i32, dbl, dbl, C.c_int, vp]
         L.aw_stage_constants.argtypes = [C.c_int, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
@@ -152,7 +160,7 @@ def aw_common_tangent(seed):
 class Ensemble:
     """Caller-owned SoA planes (torch CUDA tensors) + the aw_state struct that points at them."""
 
-    def __init__(self, n, tangent=True, wind=True, order=4, device="cuda:0"):
+    def __init__(self, n, tangent=True, wind=True, order=4, device="cuda:0", ref=False):
         _, pitch = aw_state_bytes(n, tangent, wind)
         self.n, self.pitch = int(n), pitch
         dev = torch.device(device)
@@ -165,12 +173,27 @@ class Ensemble:
         self.c = AwState(n, pitch, self.q.data_ptr(), self.w.data_ptr() if tangent else None,
                          self.acc.data_ptr(), self.wind.data_ptr() if wind else None,
                          self.status.data_ptr(), float("nan"), float("nan"), 0.0, 0, order, 0, 0, 0, None)
+        # snapshot planes for aw_mark (window start of P:67 / P(0) of P:37); allocated on request
+        self.qref = torch.zeros((6, pitch), dtype=torch.float64, device=dev) if ref else None
+        self.windref = torch.zeros((3, pitch), dtype=torch.int32, device=dev) if (ref and wind) else None
+        if ref:
+            self.c.qref = self.qref.data_ptr()
+            self.c.windref = self.windref.data_ptr() if wind else None
 
     # plain-data views of the struct
     E = property(lambda s: s.c.E)
     eps = property(lambda s: s.c.eps)
     t = property(lambda s: s.c.t)
     step = property(lambda s: s.c.step)
+    tref = property(lambda s: s.c.tref)
+
+    def set_survivors(self, rect):
+        """rect = (lo_x, hi_x, lo_y, hi_y) switches the survivor filter of P:99 on; None switches it off."""
+        if rect is None:
+            self.c.survive = 0
+        else:
+            self.c.survive = 1
+            self.c.surv_lo_x, self.c.surv_hi_x, self.c.surv_lo_y, self.c.surv_hi_y = rect
 
     @property
     def order(self):
@@ -212,6 +235,12 @@ def aw_init_shell(ens, grid, E, eps, seed, stream=None):
 def aw_integrate(ens, n, steps, dt, stride, stream=None):
     ens.bind_stream(stream)
     _check(lib().aw_integrate(C.byref(ens.c), n, steps, dt, stride), "aw_integrate")
+    return ens
+
+
+def aw_mark(ens, stream=None):
+    ens.bind_stream(stream)
+    _check(lib().aw_mark(C.byref(ens.c)), "aw_mark")
     return ens
 
 

@@ -151,10 +151,23 @@ static int check_planes(const aw_state *s) {
   if (s->n > 0) {
     if (!s->q || !s->acc || !s->status) return AW_EINVAL;
     if (!aligned16(s->q) || !aligned16(s->acc) || (s->w && !aligned16(s->w)) ||
-        (s->wind && !aligned16(s->wind)))
+        (s->wind && !aligned16(s->wind)) || (s->qref && !aligned16(s->qref)) ||
+        (s->windref && !aligned16(s->windref)))
       return AW_EINVAL;
   }
   return AW_OK;
+}
+
+// the marked snapshot is usable: planes present, wind/windref paired
+static bool has_ref(const aw_state *s) { return s->qref && ((s->wind == nullptr) == (s->windref == nullptr)); }
+
+static VelocityArgs velocity_args(const aw_state *s) {
+  VelocityArgs v;
+  v.q = s->q; v.qref = s->qref; v.wind = s->wind; v.windref = s->windref;
+  v.pitch = s->pitch;
+  v.Dt = s->t - s->tref;
+  v.radius = std::sqrt(2.0 * s->E);
+  return v;
 }
 
 }  // namespace aw
@@ -230,7 +243,7 @@ int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps, uint64
   } else if (grid->shape == AW_SHAPE_DISK || grid->shape == AW_SHAPE_GAUSS) {
     if (!(grid->r >= 0.0) || !std::isfinite(grid->r) || !std::isfinite(grid->cx) || !std::isfinite(grid->cy))
       return AW_EINVAL;
-  } else {
+  } else if (grid->shape != AW_SHAPE_SPHERE) {
     return AW_EINVAL;
   }
   if (!std::isfinite(E) || !std::isfinite(eps) || !(E - 2.0 * std::fabs(eps) > 0.0)) return AW_ERANGE;
@@ -277,6 +290,10 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
   p.a2_first = 2.0 * p.a_first; p.a2_merge = 2.0 * p.a_merge; p.a2_last = 2.0 * p.a_last;
   for (int k = 0; k < kMaxStages; ++k) p.a2_mid[k] = 2.0 * p.a_mid[k];
   p.eps = s->eps;
+  if (s->survive != 0 && s->survive != 1) return AW_EINVAL;
+  p.survive = s->survive;
+  p.surv[0] = s->surv_lo_x; p.surv[1] = s->surv_hi_x; p.surv[2] = s->surv_lo_y; p.surv[3] = s->surv_hi_y;
+  if (s->survive && !(s->surv_hi_x > s->surv_lo_x && s->surv_hi_y > s->surv_lo_y)) return AW_EINVAL;
   // running-(sin, cos) variant: degree from the largest drift angle, re-synchronisation cadence from stride
   double amax = std::fabs(p.a_first);
   amax = std::fmax(amax, std::fmax(std::fabs(p.a_merge), std::fabs(p.a_last)));
@@ -301,12 +318,37 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
   return AW_OK;
 }
 
+int aw_mark(aw_state *s) {
+  if (!s) return AW_EINVAL;
+  int rc = check_planes(s);
+  if (rc != AW_OK) return rc;
+  if (!s->ready) return AW_ESTATE;
+  if (s->n > 0 && !has_ref(s)) return AW_ESTATE;
+  cudaStream_t st = (cudaStream_t)s->stream;
+  if (s->n > 0) {
+    AW_CUDA(cudaMemcpyAsync(s->qref, s->q, (size_t)6 * s->pitch * 8, cudaMemcpyDeviceToDevice, st));
+    if (s->wind)
+      AW_CUDA(cudaMemcpyAsync(s->windref, s->wind, (size_t)3 * s->pitch * 4, cudaMemcpyDeviceToDevice, st));
+  }
+  s->tref = s->t;
+  return AW_OK;
+}
+
 int aw_indicator(const aw_state *s, int kind, double thr, void *out_dev) {
   if (!s || !out_dev) return AW_EINVAL;
   int rc = check_planes(s);
   if (rc != AW_OK) return rc;
-  if (kind < AW_IND_FLI || kind > AW_IND_CLASS) return AW_EINVAL;
+  if (kind < AW_IND_FLI || kind > AW_IND_VZ) return AW_EINVAL;
   if (!s->ready) return AW_ESTATE;
+  if (kind >= AW_IND_DP) {
+    if (!has_ref(s)) return AW_ESTATE;
+    if (kind != AW_IND_DP && !(s->t > s->tref)) return AW_ESTATE;
+    if (!aligned16(out_dev)) return AW_EINVAL;
+    if (s->n == 0) return AW_OK;
+    AW_CUDA(launch_indicator_ref(velocity_args(s), s->status, s->n, kind, static_cast<double *>(out_dev),
+                                 (cudaStream_t)s->stream));
+    return AW_OK;
+  }
   if (kind != AW_IND_DH && !s->w) return AW_ESTATE;
   if (kind == AW_IND_FTLE && !(s->t > 0.0)) return AW_ESTATE;
   if (kind == AW_IND_CLASS && thr != thr) return AW_EINVAL;
@@ -322,15 +364,16 @@ int aw_density(const aw_state *s, uint32_t *hist_dev, int32_t gx, int32_t gy, do
   if (!s || !hist_dev) return AW_EINVAL;
   int rc = check_planes(s);
   if (rc != AW_OK) return rc;
-  if (mode != 0 || gx <= 0 || gy <= 0 || !(hi > lo) || !std::isfinite(lo) || !std::isfinite(hi))
+  if (mode < AW_DENS_ACTION || mode > AW_DENS_VEL_BOTH || gx <= 0 || gy <= 0 || !(hi > lo) ||
+      !std::isfinite(lo) || !std::isfinite(hi))
     return AW_EINVAL;
   if ((int64_t)gx * gy >= 0xffffffffll) return AW_ERANGE;
   if (!s->ready) return AW_ESTATE;
+  if (mode != AW_DENS_ACTION && (!has_ref(s) || !(s->t > s->tref))) return AW_ESTATE;
   if (s->n == 0) return AW_OK;
   const double fx = (double)gx / (hi - lo), fy = (double)gy / (hi - lo);
-  AW_CUDA(launch_density(s->q + 3 * s->pitch, s->q + 4 * s->pitch, s->status, s->n, hist_dev, gx, gy, lo,
-                         fx, fy, reinterpret_cast<unsigned long long *>(dropped_dev),
-                         (cudaStream_t)s->stream));
+  AW_CUDA(launch_density(velocity_args(s), mode, s->status, s->n, hist_dev, gx, gy, lo, fx, fy,
+                         reinterpret_cast<unsigned long long *>(dropped_dev), (cudaStream_t)s->stream));
   return AW_OK;
 }
 

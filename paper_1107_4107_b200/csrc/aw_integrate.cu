@@ -203,6 +203,11 @@ __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS)
     finite = finite && isfinite(t.x) && isfinite(t.y) && isfinite(t.z) && isfinite(t.px) && isfinite(t.py) &&
              isfinite(t.pz);
     if (!finite) { status = AW_ST_NONFINITE; break; }
+    // survivor filter (R25): outside the launch rectangle at a checkpoint -> dropped, frozen here
+    if (p.survive && !(t.px >= p.surv[0] && t.px < p.surv[1] && t.py >= p.surv[2] && t.py < p.surv[3])) {
+      status = AW_ST_LEFT;
+      break;
+    }
     resync<TAN, LEVEL>(t);  // from the wrapped angles: the same values a new launch would start from
   }
 

@@ -32,6 +32,8 @@ struct IntegrateParams {
   double b2[kMaxStages];     // 2 b_s
   double b4[kMaxStages];     // 4 b_s
   double eps;
+  int32_t survive;  // survivor filter (R25): 1 = test (px, py) against surv[] at every checkpoint
+  double surv[4];   // lo_x, hi_x, lo_y, hi_y (half-open)
 };
 
 struct InitParams {
@@ -55,7 +57,19 @@ constexpr int kMaxChunk = 128;
 cudaError_t launch_init(const InitParams &p, cudaStream_t st);
 cudaError_t launch_indicator(const double *acc, const uint8_t *status, int64_t n, int64_t pitch, int kind,
                              double thr, double t, void *out, cudaStream_t st);
-cudaError_t launch_density(const double *px, const double *py, const uint8_t *status, int64_t n,
+// Everything the averaged-velocity front end needs (R26, R27): current and marked planes.
+struct VelocityArgs {
+  const double *q, *qref;          // 6*pitch each
+  const int32_t *wind, *windref;   // 3*pitch each or both NULL
+  int64_t pitch;
+  double Dt;      // t - tref > 0
+  double radius;  // sqrt(2E), rounded once on the host
+};
+// kinds AW_IND_DP, AW_IND_VX..VZ
+cudaError_t launch_indicator_ref(const VelocityArgs &v, const uint8_t *status, int64_t n, int kind, double *out,
+                                 cudaStream_t st);
+// mode 0: bins (px, py) = planes 3, 4 of v.q; modes 1-3: bins (Vhat_x, Vhat_y) of one / both hemispheres
+cudaError_t launch_density(const VelocityArgs &v, int mode, const uint8_t *status, int64_t n,
                            uint32_t *hist, int32_t gx, int32_t gy, double lo, double fx, double fy,
                            unsigned long long *dropped, cudaStream_t st);
 cudaError_t launch_sincos_probe(const double *x, int64_t n, double *s, double *c, cudaStream_t st);

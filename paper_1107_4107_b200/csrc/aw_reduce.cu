@@ -30,6 +30,57 @@ __global__ void __launch_bounds__(256) indicator_kernel(const double *__restrict
   static_cast<double *>(out)[k] = v;
 }
 
+// ---------------------------------------------------------------------- §8(f) 1-2: the paper's indicator
+// Averaged finite-time velocity over the window since aw_mark and its central projection on S (P:67,
+// P:171 fn. 26; R26, R27).  Every operation is rounded separately, in the order include/aw.h states (the
+// explicit-rounding intrinsics stop the compiler from contracting them into FMAs), so that the bin a
+// point falls in is decided by the same fp64 numbers on both sides of the parity test.
+constexpr double kTwoPiHi = 6.283185307179586;  // double nearest 2 pi
+
+__device__ __forceinline__ bool averaged_velocity(const VelocityArgs &v, int64_t k, double vh[3]) {
+  double V[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const double dxw = __dsub_rn(v.q[a * v.pitch + k], v.qref[a * v.pitch + k]);
+    const int dk = v.wind ? v.wind[a * v.pitch + k] - v.windref[a * v.pitch + k] : 0;
+    const double dX = __dadd_rn(__dmul_rn((double)dk, kTwoPiHi), dxw);
+    V[a] = __ddiv_rn(dX, v.Dt);
+  }
+  double n2 = __dmul_rn(V[0], V[0]);
+  n2 = __dadd_rn(n2, __dmul_rn(V[1], V[1]));
+  n2 = __dadd_rn(n2, __dmul_rn(V[2], V[2]));
+  const double nrm = __dsqrt_rn(n2);
+  if (!(nrm > 0.0) || !isfinite(nrm)) return false;
+  const double scale = __ddiv_rn(v.radius, nrm);
+#pragma unroll
+  for (int a = 0; a < 3; ++a) vh[a] = __dmul_rn(V[a], scale);
+  return true;
+}
+
+__global__ void __launch_bounds__(256) indicator_ref_kernel(const __grid_constant__ VelocityArgs v,
+                                                            const uint8_t *__restrict__ status, int64_t n,
+                                                            int kind, double *__restrict__ out) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  double r = __longlong_as_double(0x7ff8000000000000ll);
+  if (status[k] == AW_ST_LIVE) {
+    if (kind == AW_IND_DP) {  // |P(t) - P(0)|
+      const int64_t P = v.pitch;
+      const double d0 = __dsub_rn(v.q[3 * P + k], v.qref[3 * P + k]);
+      const double d1 = __dsub_rn(v.q[4 * P + k], v.qref[4 * P + k]);
+      const double d2 = __dsub_rn(v.q[5 * P + k], v.qref[5 * P + k]);
+      double s2 = __dmul_rn(d0, d0);
+      s2 = __dadd_rn(s2, __dmul_rn(d1, d1));
+      s2 = __dadd_rn(s2, __dmul_rn(d2, d2));
+      r = __dsqrt_rn(s2);
+    } else {
+      double vh[3];
+      if (averaged_velocity(v, k, vh)) r = kind == AW_IND_VX ? vh[0] : (kind == AW_IND_VY ? vh[1] : vh[2]);
+    }
+  }
+  out[k] = r;
+}
+
 // ------------------------------------------------------------------------------------------- a6
 // The histogram (1024 x 1024 uint32 = 4 MiB at configs[4]) does not fit in shared memory, so the
 // privatisation is a per-block open-addressing table of (bin, count) pairs in shared memory:
@@ -46,8 +97,10 @@ constexpr int kDensityBlock = 256;
 constexpr int kItems = 16;  // points per thread
 constexpr unsigned kEmpty = 0xffffffffu;
 
+// MODE 0: the point is the instantaneous (px, py); MODE 1: (Vhat_x, Vhat_y), hemisphere chosen by `hemi`.
+template <int MODE>
 __global__ void __launch_bounds__(kDensityBlock)
-    density_kernel(const double *__restrict__ px, const double *__restrict__ py,
+    density_kernel(const __grid_constant__ VelocityArgs v, int hemi,
                    const uint8_t *__restrict__ status, int64_t n, uint32_t *hist, int32_t gx, int32_t gy,
                    double lo, double fx, double fy, unsigned long long *dropped) {
   __shared__ unsigned keys[kTable];
@@ -65,10 +118,25 @@ __global__ void __launch_bounds__(kDensityBlock)
     const int64_t k = base + (int64_t)it * kDensityBlock + threadIdx.x;  // warp-uniform trip count
     unsigned bin = kEmpty;
     if (k < n && status[k] == AW_ST_LIVE) {
-      const double ax = floor(__dmul_rn(__dsub_rn(px[k], lo), fx));
-      const double ay = floor(__dmul_rn(__dsub_rn(py[k], lo), fy));
-      if (ax >= 0.0 && ax < dgx && ay >= 0.0 && ay < dgy) bin = (unsigned)((int64_t)ay * gx + (int64_t)ax);
-      else ++my_dropped;
+      double bx, by;
+      bool in = true;
+      if (MODE == 0) {
+        bx = v.q[3 * v.pitch + k];
+        by = v.q[4 * v.pitch + k];
+      } else {
+        double vh[3];
+        in = averaged_velocity(v, k, vh);
+        if (in) in = (hemi == AW_DENS_VEL_BOTH) || (hemi == AW_DENS_VEL_UPPER ? vh[2] >= 0.0 : vh[2] < 0.0);
+        bx = vh[0];
+        by = vh[1];
+      }
+      if (in) {
+        const double ax = floor(__dmul_rn(__dsub_rn(bx, lo), fx));
+        const double ay = floor(__dmul_rn(__dsub_rn(by, lo), fy));
+        in = ax >= 0.0 && ax < dgx && ay >= 0.0 && ay < dgy;
+        if (in) bin = (unsigned)((int64_t)ay * gx + (int64_t)ax);
+      }
+      if (!in) ++my_dropped;
     }
     const unsigned peers = __match_any_sync(0xffffffffu, bin);
     if (bin != kEmpty && (__ffs(peers) - 1) == (int)(threadIdx.x & 31)) {
@@ -123,12 +191,22 @@ cudaError_t launch_indicator(const double *acc, const uint8_t *status, int64_t n
   return cudaGetLastError();
 }
 
-cudaError_t launch_density(const double *px, const double *py, const uint8_t *status, int64_t n,
+cudaError_t launch_indicator_ref(const VelocityArgs &v, const uint8_t *status, int64_t n, int kind, double *out,
+                                 cudaStream_t st) {
+  indicator_ref_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(v, status, n, kind, out);
+  count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_density(const VelocityArgs &v, int mode, const uint8_t *status, int64_t n,
                            uint32_t *hist, int32_t gx, int32_t gy, double lo, double fx, double fy,
                            unsigned long long *dropped, cudaStream_t st) {
   const int64_t per_block = (int64_t)kDensityBlock * kItems;
-  density_kernel<<<(unsigned)((n + per_block - 1) / per_block), kDensityBlock, 0, st>>>(
-      px, py, status, n, hist, gx, gy, lo, fx, fy, dropped);
+  const unsigned blocks = (unsigned)((n + per_block - 1) / per_block);
+  if (mode == AW_DENS_ACTION)
+    density_kernel<0><<<blocks, kDensityBlock, 0, st>>>(v, mode, status, n, hist, gx, gy, lo, fx, fy, dropped);
+  else
+    density_kernel<1><<<blocks, kDensityBlock, 0, st>>>(v, mode, status, n, hist, gx, gy, lo, fx, fy, dropped);
   count_launch();
   return cudaGetLastError();
 }

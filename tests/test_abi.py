@@ -31,7 +31,7 @@ def test_library_exports_every_declared_symbol(aw):
     L = C.CDLL(os.path.join(ROOT, "paper_1107_4107_b200", "libaw.so"))
     for n in names:
         assert hasattr(L, n), n
-    assert aw.aw_version() == 100
+    assert aw.aw_version() == 110
     assert aw.aw_strerror(0) == "ok" and "invalid" in aw.aw_strerror(-1)
 
 
@@ -126,7 +126,21 @@ def test_validation_happens_on_the_host(aw):
     assert L.aw_indicator(C.byref(st), 9, 0.0, base) == EINVAL
     assert L.aw_indicator(C.byref(st), 2, 0.0, None) == EINVAL
     assert L.aw_density(C.byref(st), base, 16, 16, 1.0, -1.0, 0, None) == EINVAL
-    assert L.aw_density(C.byref(st), base, 16, 16, -1.0, 1.0, 1, None) == EINVAL   # mode 1 not built
+    assert L.aw_density(C.byref(st), base, 16, 16, -1.0, 1.0, 4, None) == EINVAL   # no such mode
+    assert L.aw_density(C.byref(st), base, 16, 16, -1.0, 1.0, 1, None) == ESTATE   # velocity mode, no snapshot
+    assert L.aw_indicator(C.byref(st), 4, 0.0, base) == ESTATE              # dP without a snapshot
+    assert L.aw_mark(C.byref(st)) == ESTATE                                 # no qref planes
+    st.qref = base
+    st.tref, st.t = 0.0, 0.0
+    assert L.aw_density(C.byref(st), base, 16, 16, -1.0, 1.0, 1, None) == ESTATE   # empty window t == tref
+    assert L.aw_indicator(C.byref(st), 5, 0.0, base) == ESTATE
+    st.qref = None
+    # survivor filter: flag must be 0/1 and the rectangle non-empty
+    st.survive = 2
+    assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == EINVAL
+    st.survive, st.surv_lo_x, st.surv_hi_x, st.surv_lo_y, st.surv_hi_y = 1, 0.5, 0.5, -1.0, 1.0
+    assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == EINVAL
+    st.survive = 0
     assert L.aw_density(C.byref(st), None, 16, 16, -1.0, 1.0, 0, None) == EINVAL
     assert L.aw_density(C.byref(st), base, 0, 16, -1.0, 1.0, 0, None) == EINVAL
     # zero-size ensemble: every call is a no-op that never reaches the device

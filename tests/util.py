@@ -20,6 +20,12 @@ def ensemble_to_oracle(ens, orc):
         st.wind[:] = ens.wind.cpu().numpy()
     st.status[:] = ens.status[:ens.n].cpu().numpy()
     st.E, st.eps, st.t, st.step, st.order = ens.E, ens.eps, ens.t, ens.step, ens.order
+    if getattr(ens, "qref", None) is not None:           # snapshot of aw_mark (window start)
+        st.qref = ens.qref.cpu().numpy().copy()
+        st.windref = None if ens.windref is None else ens.windref.cpu().numpy().copy()
+        st.tref = ens.tref
+    if ens.c.survive:
+        st.surv = (ens.c.surv_lo_x, ens.c.surv_hi_x, ens.c.surv_lo_y, ens.c.surv_hi_y)
     return st
 
 
