@@ -143,6 +143,20 @@ static void common_tangent(uint64_t seed, double t[6]) {
   for (int i = 0; i < 6; ++i) t[i] = t[i] / nu;
 }
 
+// Coefficients of the drift rotation by the angle d = A p as polynomials in z = p^2 (aw_internal.cuh):
+// G[i] = (-1)^i A^(2i+1)/(2i+1)!  (G[0] = A exactly),  M[i] = (-1)^(i+1) A^(2i+2)/(2i+2)!; evaluated in long
+// double and rounded once.
+static void rotation_coefficients(double A, double G[kTrigTerms + 1], double M[kTrigTerms]) {
+  const long double a = (long double)A, a2 = a * a;
+  long double pw = a, fact = 1.0L;  // pw = A^(2i+1), fact = (2i+1)!
+  for (int i = 0; i <= kTrigTerms; ++i) {
+    if (i > 0) { pw *= a2; fact *= (long double)(2 * i) * (long double)(2 * i + 1); }
+    G[i] = (double)((i & 1 ? -pw : pw) / fact);
+    if (i < kTrigTerms) M[i] = (double)((i & 1 ? pw : -pw) * a / (fact * (long double)(2 * i + 2)));
+  }
+  G[0] = A;
+}
+
 static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 static int check_planes(const aw_state *s) {
@@ -282,22 +296,25 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
   p.q = s->q; p.w = s->w; p.acc = s->acc; p.wind = s->wind; p.status = s->status;
   p.n = s->n; p.pitch = s->pitch;
   p.stride = (int32_t)stride;
-  p.a_first = a[0];
-  p.a_last = a[S];
-  p.a_merge = a[S] + a[0];
-  for (int k = 1; k < S; ++k) p.a_mid[k - 1] = a[k];
+  // palindromic stage lists (order 4 and 6): a_1 == a_{S+1}, so the merged drift a_{S+1} + a_1 = 2 a_1 exactly
+  if (a[0] != a[S]) return AW_ESTATE;
+  p.a_open = a[0];
+  for (int k = 1; k < S; ++k) p.a_loop[k - 1] = a[k];
+  p.a_loop[S - 1] = a[S] + a[0];
   for (int k = 0; k < S; ++k) { p.b1[k] = b[k]; p.b2[k] = 2.0 * b[k]; p.b4[k] = 4.0 * b[k]; }
-  p.a2_first = 2.0 * p.a_first; p.a2_merge = 2.0 * p.a_merge; p.a2_last = 2.0 * p.a_last;
-  for (int k = 0; k < kMaxStages; ++k) p.a2_mid[k] = 2.0 * p.a_mid[k];
+  for (int k = 0; k < S; ++k) {
+    p.a2_loop[k] = 2.0 * p.a_loop[k];
+    rotation_coefficients(p.a_loop[k], p.gxy[k], p.mxy[k]);
+    rotation_coefficients(2.0 * p.a_loop[k], p.gz[k], p.mz[k]);
+  }
   p.eps = s->eps;
   if (s->survive != 0 && s->survive != 1) return AW_EINVAL;
   p.survive = s->survive;
   p.surv[0] = s->surv_lo_x; p.surv[1] = s->surv_hi_x; p.surv[2] = s->surv_lo_y; p.surv[3] = s->surv_hi_y;
   if (s->survive && !(s->surv_hi_x > s->surv_lo_x && s->surv_hi_y > s->surv_lo_y)) return AW_EINVAL;
   // running-(sin, cos) variant: degree from the largest drift angle, re-synchronisation cadence from stride
-  double amax = std::fabs(p.a_first);
-  amax = std::fmax(amax, std::fmax(std::fabs(p.a_merge), std::fabs(p.a_last)));
-  for (int k = 0; k + 1 < S; ++k) amax = std::fmax(amax, std::fabs(p.a_mid[k]));
+  double amax = std::fabs(p.a_open);
+  for (int k = 0; k < S; ++k) amax = std::fmax(amax, std::fabs(p.a_loop[k]));
   p.level = s->trig ? 0 : trig_level_for(amax * vmax);
   const int64_t pieces = (stride + kMaxChunk - 1) / kMaxChunk;
   p.chunk = (int32_t)((stride + pieces - 1) / pieces);

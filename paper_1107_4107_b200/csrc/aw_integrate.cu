@@ -7,18 +7,27 @@
 //
 // Scheme (ref. 25; R2): for s = 1..S { X += a_s P ; P -= b_s grad H_p(X) }  X += a_{S+1} P.
 // Inside a block of `stride` steps the closing drift of a step and the opening drift of the next are
-// one FMA with the constant a_{S+1} + a_1 (same map, one rounding fewer; DESIGN.md §7 D3).
+// one FMA with the constant a_{S+1} + a_1 (same map, one rounding fewer; DESIGN.md §7 D3).  A block is
+//   X += a_1 P;  stride x { for s: kick_s; X += a_loop[s] P };  X -= a_1 P;  checkpoint
+// (a_1 = a_{S+1} for the palindromic stage lists, so the last merged drift minus a_1 P is the closing drift).
 // Model (eq. 2) with F = 1 + cos 2z:  H_p = cx cy F,
 //   grad H_p = (-sx cy F, -cx sy F, -2 cx cy sin 2z),  Hessian in SURVEY.md Appendix A.2.
 //
 // Trigonometry.  LEVEL 0: the device sincos (aw_trig.cuh) of x, y, z at every stage.
 // LEVEL >= 1: the pairs (sin x, cos x), (sin y, cos y), (sin 2z, cos 2z) are carried in registers and
 // advanced through every drift X += a P by the rotation with the drift angle d = a p (2 a pz for 2z):
-//     s' = s + (s m + c g),  c' = c + (c m - s g),   g = sin d,  m = cos d - 1,
-// g and m being Taylor polynomials in d whose degree the host picks from the largest possible |d| so
-// that the truncation error stays below 2^-60 (trig_level_for).  The pairs are re-synchronised from the
-// tracked angles with the full sincos at every checkpoint and at least every kMaxChunk steps, which
-// bounds the rounding random walk of the rotations at a few 1e-15.
+//     s' = s + (s m + c g),  c' = c + (c m - s g),   g = sin d = p G(p^2),  m = cos d - 1 = p^2 M(p^2),
+// G and M being the Taylor polynomials of sin and cos - 1 with the powers of a folded into their
+// coefficients on the host (constant-bank operands); the degree is picked on the host from the largest
+// possible |d| so that the truncation error stays below 2^-60 (trig_level_for).  The pairs are
+// re-synchronised from the tracked angles with the full sincos after the opening drift of every block and
+// at least every kMaxChunk steps, which bounds the rounding random walk of the rotations at a few 1e-15.
+//
+// Instruction shapes (profiles/r1c_dfma_operands.md): on sm_100 a DFMA that reads three distinct 64-bit
+// registers issues every 3 cycles instead of 2 unless one operand comes from the operand-reuse cache, the
+// constant bank or an immediate.  The code below therefore keeps polynomial coefficients and stage
+// constants in the constant bank and writes the remaining three-register FMAs in groups that share an
+// operand in the same slot (the rotation's g, the kick's F, the tangent map's column vector).
 #include <cmath>
 
 #include "aw_internal.cuh"
@@ -46,28 +55,46 @@ __device__ __forceinline__ double wrap_angle(double x, int &turns) {
   return fma(-k, kTwoPiLo, fma(-k, kTwoPiHi, x));
 }
 
-// g = sin d, m = cos d - 1 for a small angle d: Taylor series with N terms beyond the leading one.
-// Truncation: |d|^(2N+3)/(2N+3)! in g, |d|^(2N+2)/(2N+2)! in m.  N + N FMA + 3 DMUL.
+// g = sin(A p), m = cos(A p) - 1 as p G(z), z M(z), z = p^2: N + (N-1) FMA with constant-bank coefficients,
+// 3 DMUL.  Truncation: |d|^(2N+3)/(2N+3)! in g, |d|^(2N+2)/(2N+2)! in m (d = A p).
 template <int N>
-__device__ __forceinline__ void small_sincos(double d, double &g, double &m) {
-  constexpr double S[5] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0, -1.0 / 39916800.0};
-  constexpr double C[5] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0, -1.0 / 3628800.0};
+__device__ __forceinline__ void small_sincos(double p, const double (&G)[kTrigTerms + 1],
+                                             const double (&M)[kTrigTerms], double &g, double &m) {
+  static_assert(N >= 1 && N <= kTrigTerms, "degree");
+  const double z = p * p;
+  double pg = G[N], pm = M[N - 1];
+#pragma unroll
+  for (int i = N - 1; i >= 0; --i) pg = fma(pg, z, G[i]);
+#pragma unroll
+  for (int i = N - 2; i >= 0; --i) pm = fma(pm, z, M[i]);
+  g = p * pg;
+  m = z * pm;
+}
+
+// The same two functions of the angle d itself, with the universal Taylor coefficients: used by the 7-stage
+// scheme, whose four distinct drift constants would otherwise need four sets of leading coefficients in
+// registers (a DFMA takes one constant-bank operand at most).  N + (N-1) FMA, 3 DMUL, plus d = A p outside.
+template <int N>
+__device__ __forceinline__ void small_sincos_angle(double d, double &g, double &m) {
+  constexpr double Sc[5] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0, -1.0 / 39916800.0};
+  constexpr double Cc[5] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0, -1.0 / 3628800.0};
   static_assert(N >= 1 && N <= 5, "degree");
   const double z = d * d;
-  double ps = S[N - 1], pc = C[N - 1];
+  double pg = Sc[N - 1], pm = Cc[N - 1];
 #pragma unroll
   for (int i = N - 2; i >= 0; --i) {
-    ps = fma(ps, z, S[i]);
-    pc = fma(pc, z, C[i]);
+    pg = fma(pg, z, Sc[i]);
+    pm = fma(pm, z, Cc[i]);
   }
-  g = fma(d * z, ps, d);
-  m = z * pc;
+  pg = fma(pg, z, 1.0);
+  g = d * pg;
+  m = z * pm;
 }
 
 // (s, c) <- rotation of (s, c) by the angle whose sine is g and cosine is 1 + m; <= 1 ulp each.
 __device__ __forceinline__ void rotate(double &s, double &c, double g, double m) {
-  const double s1 = fma(c, g, fma(s, m, s));
-  const double c1 = fma(-s, g, fma(c, m, c));
+  const double t1 = fma(s, m, s), t2 = fma(c, m, c);
+  const double s1 = fma(c, g, t1), c1 = fma(-s, g, t2);
   s = s1;
   c = c1;
 }
@@ -88,19 +115,38 @@ struct Traj {
   double sx, cx, sy, cy, s2, c2;  // sin x, cos x, sin y, cos y, sin 2z, cos 2z (LEVEL >= 1)
 };
 
-template <bool TAN, int LEVEL>
-__device__ __forceinline__ void drift(Traj<TAN> &t, double a, double a2) {
-  if (LEVEL > 0) {
-    double g, m;
-    small_sincos<Deg<LEVEL>::xy>(a * t.px, g, m);
-    rotate(t.sx, t.cx, g, m);
-    small_sincos<Deg<LEVEL>::xy>(a * t.py, g, m);
-    rotate(t.sy, t.cy, g, m);
-    small_sincos<Deg<LEVEL>::z>(a2 * t.pz, g, m);
-    rotate(t.s2, t.c2, g, m);
-  }
+// angles (and tangent angles) only: X += a P
+template <bool TAN>
+__device__ __forceinline__ void drift_angles(Traj<TAN> &t, double a) {
   t.x = fma(a, t.px, t.x); t.y = fma(a, t.py, t.y); t.z = fma(a, t.pz, t.z);
   if (TAN) { t.dx = fma(a, t.dpx, t.dx); t.dy = fma(a, t.dpy, t.dy); t.dz = fma(a, t.dpz, t.dz); }
+}
+
+// drift after kick s of the step loop: angles and, for LEVEL >= 1, the running pairs.  The stage lists are
+// palindromic, so a_loop[s] == a_loop[S-2-s] for s < S-1: both use the coefficient set of the smaller index
+// (fewer distinct constants for the compiler to keep at hand).
+template <int S, bool TAN, int LEVEL, int s>
+__device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
+  constexpr int cs = (s == S - 1) ? s : (s < S - 2 - s ? s : S - 2 - s);
+  if (LEVEL > 0) {
+    double g, m;
+    if (S <= 3) {
+      small_sincos<Deg<LEVEL>::xy>(t.px, p.gxy[cs], p.mxy[cs], g, m);
+      rotate(t.sx, t.cx, g, m);
+      small_sincos<Deg<LEVEL>::xy>(t.py, p.gxy[cs], p.mxy[cs], g, m);
+      rotate(t.sy, t.cy, g, m);
+      small_sincos<Deg<LEVEL>::z>(t.pz, p.gz[cs], p.mz[cs], g, m);
+      rotate(t.s2, t.c2, g, m);
+    } else {
+      small_sincos_angle<Deg<LEVEL>::xy>(p.a_loop[cs] * t.px, g, m);
+      rotate(t.sx, t.cx, g, m);
+      small_sincos_angle<Deg<LEVEL>::xy>(p.a_loop[cs] * t.py, g, m);
+      rotate(t.sy, t.cy, g, m);
+      small_sincos_angle<Deg<LEVEL>::z>(p.a2_loop[cs] * t.pz, g, m);
+      rotate(t.s2, t.c2, g, m);
+    }
+  }
+  drift_angles<TAN>(t, p.a_loop[cs]);
 }
 
 template <bool TAN, int LEVEL>
@@ -130,13 +176,24 @@ __device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2, double 
   t.py = fma(cs, F, t.py);
   t.pz = fma(c, G, t.pz);
   if (TAN) {
-    // rows of -b Hess H_p: (e1,-e2,-e3), (-e2,e1,-e4), (-e3,-e4,e5)
+    // rows of -b Hess H_p: (e1,-e2,-e3), (-e2,e1,-e4), (-e3,-e4,e5); applied column by column so that
+    // consecutive FMAs share the tangent component (operand-reuse cache) and are independent
     const double ss = t.sx * t.sy;
     const double e1 = c * F, e2 = ss * F, e3 = sc * G, e4 = cs * G;
     const double e5 = c * (b4 * t.c2);  // 4 b cx cy cos 2z
-    t.dpx = fma(e1, t.dx, t.dpx); t.dpx = fma(-e2, t.dy, t.dpx); t.dpx = fma(-e3, t.dz, t.dpx);
-    t.dpy = fma(e1, t.dy, t.dpy); t.dpy = fma(-e2, t.dx, t.dpy); t.dpy = fma(-e4, t.dz, t.dpy);
-    t.dpz = fma(e5, t.dz, t.dpz); t.dpz = fma(-e3, t.dx, t.dpz); t.dpz = fma(-e4, t.dy, t.dpz);
+    t.dpx = fma(e1, t.dx, t.dpx); t.dpy = fma(-e2, t.dx, t.dpy); t.dpz = fma(-e3, t.dx, t.dpz);
+    t.dpx = fma(-e2, t.dy, t.dpx); t.dpy = fma(e1, t.dy, t.dpy); t.dpz = fma(-e4, t.dy, t.dpz);
+    t.dpx = fma(-e3, t.dz, t.dpx); t.dpy = fma(-e4, t.dz, t.dpy); t.dpz = fma(e5, t.dz, t.dpz);
+  }
+}
+
+// stages s, s+1, ..., S-1 of one step: kick_s then the drift after it
+template <int S, bool TAN, int LEVEL, int s>
+__device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p) {
+  if constexpr (s < S) {
+    kick<TAN, LEVEL>(t, p.b1[s], p.b2[s], p.b4[s]);
+    drift<S, TAN, LEVEL, s>(t, p);
+    stages<S, TAN, LEVEL, s + 1>(t, p);
   }
 }
 
@@ -155,28 +212,21 @@ __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS)
     t.dx = p.w[k]; t.dy = p.w[P + k]; t.dz = p.w[2 * P + k];
     t.dpx = p.w[3 * P + k]; t.dpy = p.w[4 * P + k]; t.dpz = p.w[5 * P + k];
   }
-  resync<TAN, LEVEL>(t);
   int status = AW_ST_LIVE;
 
   for (int chk = 0; chk < p.nchk; ++chk) {
-    drift<TAN, LEVEL>(t, p.a_first, p.a2_first);  // opening drift of the block
+    drift_angles<TAN>(t, p.a_open);  // opening drift of the block
+    resync<TAN, LEVEL>(t);           // pairs from the angles: the same values a new launch would start from
 
 #pragma unroll 1
     for (int rem = p.stride; rem > 0;) {
       const int m = rem < p.chunk ? rem : p.chunk;
       rem -= m;
 #pragma unroll 1
-      for (int i = m; i > 0; --i) {
-#pragma unroll
-        for (int s = 0; s < S; ++s) {
-          kick<TAN, LEVEL>(t, p.b1[s], p.b2[s], p.b4[s]);
-          if (s < S - 1) drift<TAN, LEVEL>(t, p.a_mid[s], p.a2_mid[s]);
-        }
-        const bool last = (i == 1) && (rem == 0);
-        drift<TAN, LEVEL>(t, last ? p.a_last : p.a_merge, last ? p.a2_last : p.a2_merge);
-      }
+      for (int i = m; i > 0; --i) stages<S, TAN, LEVEL, 0>(t, p);
       if (rem > 0) resync<TAN, LEVEL>(t);
     }
+    drift_angles<TAN>(t, -p.a_open);  // last merged drift -> closing drift of the block
 
     // ---- fused checkpoint (R4): (i) renormalise + log growth, (ii) energy error, (iii) wrap
     bool finite = true;
@@ -208,7 +258,6 @@ __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS)
       status = AW_ST_LEFT;
       break;
     }
-    resync<TAN, LEVEL>(t);  // from the wrapped angles: the same values a new launch would start from
   }
 
   p.q[k] = t.x; p.q[P + k] = t.y; p.q[2 * P + k] = t.z;

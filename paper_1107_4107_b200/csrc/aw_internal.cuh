@@ -8,6 +8,7 @@
 namespace aw {
 
 constexpr int kMaxStages = 7;
+constexpr int kTrigTerms = 5;  // largest Taylor degree N of the drift rotations (level 4, 2z pair)
 
 // Kernel parameters of the integrator; lives in the constant bank (__grid_constant__), so the stage
 // constants are constant-bank operands of the DFMA instructions and cost no registers.
@@ -23,11 +24,17 @@ struct IntegrateParams {
   int32_t chunk;   // steps between re-synchronisations of the running (sin, cos) pairs; divides the
                    // stride into equal-as-possible pieces of <= kMaxChunk steps (a function of stride only)
   int32_t level;   // trigonometry variant picked on the host from the largest drift angle (aw_integrate.cu)
-  double a_first;  // a_1: drift that opens a block of `stride` steps
-  double a_merge;  // a_{S+1} + a_1: closing drift of one step merged with the opening drift of the next
-  double a_last;   // a_{S+1}: drift that closes the block
-  double a_mid[kMaxStages];  // a_2 .. a_S (drift after kick s, s = 1..S-1); a_mid[S-1] unused
-  double a2_first, a2_merge, a2_last, a2_mid[kMaxStages];  // twice the above (exact): drift of the angle 2z
+  double a_open;   // a_1 (= a_{S+1}): angle drift that opens a block of `stride` steps; the block is closed by
+                   // the angle drift -a_open, which takes the last merged drift back to the step boundary
+  double a2_loop[kMaxStages]; // 2 a_loop[s] (exact): drift of the angle 2z
+  double a_loop[kMaxStages];  // drift after kick s (s = 0..S-1): a_2 .. a_S, then a_{S+1} + a_1 (closing drift
+                              // of one step merged with the opening drift of the next)
+  // Rotation of the running (sin, cos) pairs through the drift after kick s by the angle d = A p, A = a_loop[s]
+  // for the x and y pairs and 2 a_loop[s] for the 2z pair, as polynomials in z = p^2 (aw_integrate.cu):
+  //   sin d = p (G[0] + G[1] z + ...),  G[i] = (-1)^i A^(2i+1) / (2i+1)!      (G[0] = A exactly)
+  //   cos d - 1 = z (M[0] + M[1] z + ...),  M[i] = (-1)^(i+1) A^(2i+2) / (2i+2)!
+  double gxy[kMaxStages][kTrigTerms + 1], mxy[kMaxStages][kTrigTerms];
+  double gz[kMaxStages][kTrigTerms + 1], mz[kMaxStages][kTrigTerms];
   double b1[kMaxStages];     // b_s
   double b2[kMaxStages];     // 2 b_s
   double b4[kMaxStages];     // 4 b_s
