@@ -150,12 +150,12 @@ AW_API int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps,
  * (the angle would leave the range the two-constant argument reduction handles exactly, R7).
  * AW_ESTATE if !s->ready or order not in {4, 6}.  Advances s->t and s->step.
  * Trigonometry: the kick needs sin/cos of x, y and 2z at every stage.  With s->trig == 0 the kernel
- * carries the three (sin, cos) pairs in registers and advances them through each drift by a rotation
+ * carries the three (sin, cos) pairs (of x + y, x - y and 2z) in registers and advances them through each drift by a rotation
  * with the drift angle d = a_s p (Taylor polynomials in d; the degree is picked on the host from
  * max_s |a_s| sqrt(2(E + 2|eps|)) so the truncation stays below 2^-60; aw_trig_level reports it), and
  * recomputes them from the angles with the device sincos at every checkpoint and at least every 128
  * steps.  s->E must therefore bound the energy of an uploaded state.  If the drift angle can exceed
- * 0.0708 rad, or with s->trig == 1, the device sincos is evaluated at every stage instead (level 0).
+ * 0.05 rad, or with s->trig == 1, the device sincos is evaluated at every stage instead (level 0).
  * The work is split into kernel launches of at most AW_MAX_STEPS_PER_LAUNCH steps (a multiple of
  * stride); the result does not depend on the split. */
 #define AW_MAX_STEPS_PER_LAUNCH 20000
@@ -201,7 +201,7 @@ AW_API int aw_density(const aw_state *s, uint32_t *hist_dev, int32_t gx, int32_t
  * four order conditions in extended precision. */
 AW_API int aw_stage_constants(int order, double dt, double eps, double *a_host, double *b_host);
 /* Trigonometry level aw_integrate would use for this state and dt: 0 = device sincos at every stage,
- * 1..4 = running pairs with Taylor degrees (x/y pair, 2z pair) = (3,3), (3,4), (4,4), (4,5); or a
+ * 1..4 = running pairs with Taylor degrees (x+y / x-y pairs, 2z pair) = (3,3), (3,4), (4,4), (4,5); or a
  * negative aw_status.  Pure host arithmetic. */
 AW_API int aw_trig_level(const aw_state *s, double dt);
 /* The common tangent vector of tangent_mode 0: unit vector from u(seed, 2^63-1, 5..10) (R12). */
@@ -247,6 +247,14 @@ AW_API int aw_hamiltonian_probe(const double *q_dev, int64_t n, int64_t pitch, d
  * (thread-instructions) to the host outputs; flop/s = 2*dfma/ms*1e3.  sink_dev: >= 8 bytes device. */
 AW_API int aw_dfma_peak_probe(int blocks, int threads, int chains, int64_t iters, double *sink_dev,
                        double *ms_host, double *dfma_host, void *stream);
+
+/* fp64 issue rate by operand shape (the register-operand bandwidth behind DESIGN.md §6.1): every thread
+ * runs 8 independent chains, 32 fp64 instructions per loop trip, `iters` trips.  shape 0: fma(v, u0, w0),
+ * two register operands shared by neighbouring instructions; 1: fma(v, u_c, w_c), three distinct registers;
+ * 2: fma(v, u_c, immediate); 3: fma(v, v, w_c); 4: v * u_c (DMUL); 5: fma(u_c, w_c', v).  Writes elapsed
+ * milliseconds and the fp64 thread-instruction count to the host outputs.  work_dev: >= 136 doubles. */
+AW_API int aw_dfma_shape_probe(int blocks, int threads, int shape, int64_t iters, double *work_dev,
+                               double *ms_host, double *inst_host, void *stream);
 
 #ifdef __cplusplus
 }

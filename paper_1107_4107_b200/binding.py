@@ -99,6 +99,7 @@ def lib():
         L.aw_hamiltonian_probe.argtypes = [vp, i64, i64, dbl, vp, vp]
         L.aw_dfma_peak_probe.argtypes = [C.c_int, C.c_int, C.c_int, i64, vp, C.POINTER(dbl),
                                          C.POINTER(dbl), vp]
+        L.aw_dfma_shape_probe.argtypes = [C.c_int, C.c_int, C.c_int, i64, vp, C.POINTER(dbl), C.POINTER(dbl), vp]
         _lib = L
     return _lib
 
@@ -302,4 +303,13 @@ def aw_dfma_peak_probe(blocks, threads, chains, iters, device="cuda:0"):
     ms, cnt = C.c_double(0), C.c_double(0)
     _check(lib().aw_dfma_peak_probe(blocks, threads, chains, iters, _ptr(sink), C.byref(ms),
                                     C.byref(cnt), _stream_ptr()), "aw_dfma_peak_probe")
+    return ms.value, cnt.value
+
+
+def aw_dfma_shape_probe(blocks, threads, shape, iters, device="cuda:0"):
+    """Returns (milliseconds, fp64 thread-instructions) for one operand shape (include/aw.h)."""
+    work = torch.zeros((160,), dtype=torch.float64, device=device)
+    ms, cnt = C.c_double(0), C.c_double(0)
+    _check(lib().aw_dfma_shape_probe(blocks, threads, shape, iters, _ptr(work), C.byref(ms), C.byref(cnt),
+                                     _stream_ptr()), "aw_dfma_shape_probe")
     return ms.value, cnt.value

@@ -301,11 +301,10 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
   p.a_open = a[0];
   for (int k = 1; k < S; ++k) p.a_loop[k - 1] = a[k];
   p.a_loop[S - 1] = a[S] + a[0];
-  for (int k = 0; k < S; ++k) { p.b1[k] = b[k]; p.b2[k] = 2.0 * b[k]; p.b4[k] = 4.0 * b[k]; }
+  for (int k = 0; k < S; ++k) { p.b1[k] = b[k]; p.b2[k] = 2.0 * b[k]; }
   for (int k = 0; k < S; ++k) {
     p.a2_loop[k] = 2.0 * p.a_loop[k];
-    rotation_coefficients(p.a_loop[k], p.gxy[k], p.mxy[k]);
-    rotation_coefficients(2.0 * p.a_loop[k], p.gz[k], p.mz[k]);
+    rotation_coefficients(p.a_loop[k], p.grot[k], p.mrot[k]);
   }
   p.eps = s->eps;
   if (s->survive != 0 && s->survive != 1) return AW_EINVAL;
@@ -484,6 +483,33 @@ int aw_dfma_peak_probe(int blocks, int threads, int chains, int64_t iters, doubl
   if (err != cudaSuccess) return cuda_fail(err);
   *ms_host = (double)ms;
   *dfma_host = (double)blocks * (double)threads * (double)chains * (double)iters;
+  return AW_OK;
+}
+
+int aw_dfma_shape_probe(int blocks, int threads, int shape, int64_t iters, double *work_dev, double *ms_host,
+                        double *inst_host, void *stream) {
+  if (blocks <= 0 || threads <= 0 || threads > 1024 || iters <= 0 || !work_dev || !ms_host || !inst_host)
+    return AW_EINVAL;
+  if (shape < 0 || shape > 5) return AW_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  double host[128];
+  for (int i = 0; i < 128; ++i) host[i] = 1.0 - 1e-9 * (double)(i % 97);
+  AW_CUDA(cudaMemcpyAsync(work_dev, host, sizeof host, cudaMemcpyHostToDevice, st));
+  cudaEvent_t e0, e1;
+  AW_CUDA(cudaEventCreate(&e0));
+  AW_CUDA(cudaEventCreate(&e1));
+  cudaError_t err = launch_dfma_shape(blocks, threads, shape, 64, work_dev + 128, work_dev, st);  // warm-up
+  if (err == cudaSuccess) err = cudaEventRecord(e0, st);
+  if (err == cudaSuccess) err = launch_dfma_shape(blocks, threads, shape, iters, work_dev + 128, work_dev, st);
+  if (err == cudaSuccess) err = cudaEventRecord(e1, st);
+  if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+  float ms = 0.f;
+  if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (err != cudaSuccess) return cuda_fail(err);
+  *ms_host = (double)ms;
+  *inst_host = (double)blocks * (double)threads * (double)iters * 32.0;
   return AW_OK;
 }
 

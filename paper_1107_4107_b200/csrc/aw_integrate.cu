@@ -99,27 +99,72 @@ __device__ __forceinline__ void rotate(double &s, double &c, double g, double m)
   c = c1;
 }
 
-// Degrees (x/y pair, 2z pair) of the trigonometry levels; the angle of the 2z pair is twice as large.
+// Degrees (u/v pairs, 2z pair) of the trigonometry levels.  With |d| = max_s |a_s| max|P| the u and v pairs see
+// angles up to sqrt(2) |d| (|px +- py| <= sqrt(2) |P|), the 2z pair up to 2 |d| (trig_level_for).
 template <int LEVEL> struct Deg;
-template <> struct Deg<0> { static constexpr int xy = 1, z = 1; };  // unused
-template <> struct Deg<1> { static constexpr int xy = 3, z = 3; };
-template <> struct Deg<2> { static constexpr int xy = 3, z = 4; };
-template <> struct Deg<3> { static constexpr int xy = 4, z = 4; };
-template <> struct Deg<4> { static constexpr int xy = 4, z = 5; };
+template <> struct Deg<0> { static constexpr int uv = 1, z = 1; };  // unused
+template <> struct Deg<1> { static constexpr int uv = 3, z = 3; };
+template <> struct Deg<2> { static constexpr int uv = 3, z = 4; };
+template <> struct Deg<3> { static constexpr int uv = 4, z = 4; };
+template <> struct Deg<4> { static constexpr int uv = 4, z = 5; };
 
-// Everything a thread carries between stages.
+// Everything a thread carries between stages.  Inside a block of `stride` steps the state is held in the
+// rotated and scaled variables
+//     u = x + y,  v = x - y,  zeta = 2 z,   pu = px + py,  pv = px - py,  pzeta = 2 pz
+// (tangent vector: du, dv, dzeta = 2 dz, dpu, dpv, and dpz itself), in which
+//     H_p = (cos u + cos v)(1 + cos zeta)/2:
+// the kick needs no products of the x and y functions,
+//     pu += b F sin u,  pv += b F sin v,  pzeta += 2 b (cos u + cos v) sin zeta,        F = 1 + cos zeta,
+// the tangent kick is seven multiply-adds instead of nine (kick()), and all three angles drift with the
+// same constant (u += a pu, v += a pv, zeta += a pzeta), so one set of rotation coefficients serves the three
+// pairs and every constant of the loop fits the uniform registers.  The change of variables is linear, so
+// the map is the same map; halving and doubling are exact; the state is converted back to (x, y, z) for
+// every checkpoint and for the store.
 template <bool TAN>
 struct Traj {
-  double x, y, z, px, py, pz;
-  double dx, dy, dz, dpx, dpy, dpz;
-  double sx, cx, sy, cy, s2, c2;  // sin x, cos x, sin y, cos y, sin 2z, cos 2z (LEVEL >= 1)
+  double u, v, zt, pu, pv, pzt;
+  double du, dv, dzt, dpu, dpv, dpz;
+  double su, cu, sv, cv, s2, c2;  // sin u, cos u, sin v, cos v, sin zeta, cos zeta (LEVEL >= 1)
 };
 
-// angles (and tangent angles) only: X += a P
+// (x, y) -> (x + y, x - y) and back, in place, for every pair of the first two degrees of freedom
+__device__ __forceinline__ void to_sum_diff(double &a, double &b) {
+  const double s = a + b, d = a - b;
+  a = s;
+  b = d;
+}
+__device__ __forceinline__ void from_sum_diff(double &a, double &b) {
+  const double x = 0.5 * (a + b), y = 0.5 * (a - b);
+  a = x;
+  b = y;
+}
 template <bool TAN>
-__device__ __forceinline__ void drift_angles(Traj<TAN> &t, double a) {
-  t.x = fma(a, t.px, t.x); t.y = fma(a, t.py, t.y); t.z = fma(a, t.pz, t.z);
-  if (TAN) { t.dx = fma(a, t.dpx, t.dx); t.dy = fma(a, t.dpy, t.dy); t.dz = fma(a, t.dpz, t.dz); }
+__device__ __forceinline__ void rotate_in(Traj<TAN> &t) {
+  to_sum_diff(t.u, t.v);
+  to_sum_diff(t.pu, t.pv);
+  t.zt *= 2.0;
+  t.pzt *= 2.0;
+  if (TAN) { to_sum_diff(t.du, t.dv); to_sum_diff(t.dpu, t.dpv); t.dzt *= 2.0; }
+}
+// The momenta come back as px = px0 + ((pu - pu0) + (pv - pv0))/2 with (px0, py0) the values the block started
+// from and pu0 = px0 + py0, pv0 = px0 - py0 as rotate_in rounded them: the differences are exact (or nearly),
+// so the rounding of the forward conversion cancels and P stays bit-constant when the kicks vanish (eps = 0).
+template <bool TAN>
+__device__ __forceinline__ void rotate_out(Traj<TAN> &t, double px0, double py0) {
+  from_sum_diff(t.u, t.v);
+  const double du = t.pu - (px0 + py0), dv = t.pv - (px0 - py0);
+  t.pu = fma(0.5, du + dv, px0);
+  t.pv = fma(0.5, du - dv, py0);
+  t.zt *= 0.5;
+  t.pzt *= 0.5;
+  if (TAN) { from_sum_diff(t.du, t.dv); from_sum_diff(t.dpu, t.dpv); t.dzt *= 0.5; }
+}
+
+// angles (and tangent angles) only: X += a P; a2 = 2a (dzeta = 2 dz advances with dpz)
+template <bool TAN>
+__device__ __forceinline__ void drift_angles(Traj<TAN> &t, double a, double a2) {
+  t.u = fma(a, t.pu, t.u); t.v = fma(a, t.pv, t.v); t.zt = fma(a, t.pzt, t.zt);
+  if (TAN) { t.du = fma(a, t.dpu, t.du); t.dv = fma(a, t.dpv, t.dv); t.dzt = fma(a2, t.dpz, t.dzt); }
 }
 
 // drift after kick s of the step loop: angles and, for LEVEL >= 1, the running pairs.  The stage lists are
@@ -131,59 +176,60 @@ __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
   if (LEVEL > 0) {
     double g, m;
     if (S <= 3) {
-      small_sincos<Deg<LEVEL>::xy>(t.px, p.gxy[cs], p.mxy[cs], g, m);
-      rotate(t.sx, t.cx, g, m);
-      small_sincos<Deg<LEVEL>::xy>(t.py, p.gxy[cs], p.mxy[cs], g, m);
-      rotate(t.sy, t.cy, g, m);
-      small_sincos<Deg<LEVEL>::z>(t.pz, p.gz[cs], p.mz[cs], g, m);
+      small_sincos<Deg<LEVEL>::uv>(t.pu, p.grot[cs], p.mrot[cs], g, m);
+      rotate(t.su, t.cu, g, m);
+      small_sincos<Deg<LEVEL>::uv>(t.pv, p.grot[cs], p.mrot[cs], g, m);
+      rotate(t.sv, t.cv, g, m);
+      small_sincos<Deg<LEVEL>::z>(t.pzt, p.grot[cs], p.mrot[cs], g, m);
       rotate(t.s2, t.c2, g, m);
     } else {
-      small_sincos_angle<Deg<LEVEL>::xy>(p.a_loop[cs] * t.px, g, m);
-      rotate(t.sx, t.cx, g, m);
-      small_sincos_angle<Deg<LEVEL>::xy>(p.a_loop[cs] * t.py, g, m);
-      rotate(t.sy, t.cy, g, m);
-      small_sincos_angle<Deg<LEVEL>::z>(p.a2_loop[cs] * t.pz, g, m);
+      small_sincos_angle<Deg<LEVEL>::uv>(p.a_loop[cs] * t.pu, g, m);
+      rotate(t.su, t.cu, g, m);
+      small_sincos_angle<Deg<LEVEL>::uv>(p.a_loop[cs] * t.pv, g, m);
+      rotate(t.sv, t.cv, g, m);
+      small_sincos_angle<Deg<LEVEL>::z>(p.a_loop[cs] * t.pzt, g, m);
       rotate(t.s2, t.c2, g, m);
     }
   }
-  drift_angles<TAN>(t, p.a_loop[cs]);
+  drift_angles<TAN>(t, p.a_loop[cs], p.a2_loop[cs]);
 }
 
 template <bool TAN, int LEVEL>
 __device__ __forceinline__ void resync(Traj<TAN> &t) {
   if (LEVEL > 0) {
-    sincos(t.x, t.sx, t.cx);
-    sincos(t.y, t.sy, t.cy);
-    sincos(2.0 * t.z, t.s2, t.c2);
+    sincos(t.u, t.su, t.cu);
+    sincos(t.v, t.sv, t.cv);
+    sincos(t.zt, t.s2, t.c2);
   }
 }
 
-// kick of stage s: P -= b grad H_p(X), dP -= b Hess H_p(X) dX (R3), b1 = b, b2 = 2b, b4 = 4b
+// kick of stage s in the rotated variables: P -= b grad H_p(X), dP -= b Hess H_p(X) dX (R3); b1 = b, b2 = 2b.
+// With F = 1 + cos zeta, W = cos u + cos v:
+//   pu += b F sin u,   pv += b F sin v,   pzeta += 2 b W sin zeta
+//   dpu += b (F cos u du - sin zeta sin u dzeta)
+//   dpv += b (F cos v dv - sin zeta sin v dzeta)
+//   dpz += b (-sin zeta (sin u du + sin v dv) + W cos zeta dzeta)
+// (the sum and difference of the x and y rows of SURVEY.md Appendix A.2, with dzeta = 2 dz).
 template <bool TAN, int LEVEL>
-__device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2, double b4) {
+__device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2) {
   if (LEVEL == 0) {
-    double sz, cz;
-    sincos(t.x, t.sx, t.cx);
-    sincos(t.y, t.sy, t.cy);
-    sincos(t.z, sz, cz);
-    t.c2 = fma(cz + cz, cz, -1.0);  // cos 2z = 2 cz^2 - 1
-    t.s2 = (sz + sz) * cz;          // sin 2z
+    sincos(t.u, t.su, t.cu);
+    sincos(t.v, t.sv, t.cv);
+    sincos(t.zt, t.s2, t.c2);
   }
-  const double F = fma(b1, t.c2, b1);  // b (1 + cos 2z)
-  const double G = b2 * t.s2;          // 2 b sin 2z
-  const double c = t.cx * t.cy, sc = t.sx * t.cy, cs = t.cx * t.sy;
-  t.px = fma(sc, F, t.px);
-  t.py = fma(cs, F, t.py);
-  t.pz = fma(c, G, t.pz);
+  const double F = fma(b1, t.c2, b1);  // b (1 + cos zeta)
+  const double G2 = b2 * t.s2;         // 2 b sin zeta
+  const double w = t.cu + t.cv;        // 2 cos x cos y
+  t.pu = fma(t.su, F, t.pu);
+  t.pv = fma(t.sv, F, t.pv);
+  t.pzt = fma(w, G2, t.pzt);
   if (TAN) {
-    // rows of -b Hess H_p: (e1,-e2,-e3), (-e2,e1,-e4), (-e3,-e4,e5); applied column by column so that
-    // consecutive FMAs share the tangent component (operand-reuse cache) and are independent
-    const double ss = t.sx * t.sy;
-    const double e1 = c * F, e2 = ss * F, e3 = sc * G, e4 = cs * G;
-    const double e5 = c * (b4 * t.c2);  // 4 b cx cy cos 2z
-    t.dpx = fma(e1, t.dx, t.dpx); t.dpy = fma(-e2, t.dx, t.dpy); t.dpz = fma(-e3, t.dx, t.dpz);
-    t.dpx = fma(-e2, t.dy, t.dpx); t.dpy = fma(e1, t.dy, t.dpy); t.dpz = fma(-e4, t.dy, t.dpz);
-    t.dpx = fma(-e3, t.dz, t.dpx); t.dpy = fma(-e4, t.dz, t.dpy); t.dpz = fma(e5, t.dz, t.dpz);
+    const double G = b1 * t.s2;  // b sin zeta
+    const double a1 = F * t.cu, a2 = F * t.cv, k1 = G * t.su, k2 = G * t.sv;
+    const double e5 = w * (b1 * t.c2);  // b (cos u + cos v) cos zeta
+    t.dpu = fma(a1, t.du, t.dpu); t.dpv = fma(a2, t.dv, t.dpv); t.dpz = fma(e5, t.dzt, t.dpz);
+    t.dpu = fma(-k1, t.dzt, t.dpu); t.dpz = fma(-k1, t.du, t.dpz);
+    t.dpv = fma(-k2, t.dzt, t.dpv); t.dpz = fma(-k2, t.dv, t.dpz);
   }
 }
 
@@ -191,7 +237,7 @@ __device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2, double 
 template <int S, bool TAN, int LEVEL, int s>
 __device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p) {
   if constexpr (s < S) {
-    kick<TAN, LEVEL>(t, p.b1[s], p.b2[s], p.b4[s]);
+    kick<TAN, LEVEL>(t, p.b1[s], p.b2[s]);
     drift<S, TAN, LEVEL, s>(t, p);
     stages<S, TAN, LEVEL, s + 1>(t, p);
   }
@@ -205,17 +251,20 @@ __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS)
   if (p.status[k] != AW_ST_LIVE) return;
   const int64_t P = p.pitch;
 
+  // between blocks the fields of t hold x, y, z, px, py, pz (and the plain tangent vector)
   Traj<TAN> t;
-  t.x = p.q[k]; t.y = p.q[P + k]; t.z = p.q[2 * P + k];
-  t.px = p.q[3 * P + k]; t.py = p.q[4 * P + k]; t.pz = p.q[5 * P + k];
+  t.u = p.q[k]; t.v = p.q[P + k]; t.zt = p.q[2 * P + k];
+  t.pu = p.q[3 * P + k]; t.pv = p.q[4 * P + k]; t.pzt = p.q[5 * P + k];
   if (TAN) {
-    t.dx = p.w[k]; t.dy = p.w[P + k]; t.dz = p.w[2 * P + k];
-    t.dpx = p.w[3 * P + k]; t.dpy = p.w[4 * P + k]; t.dpz = p.w[5 * P + k];
+    t.du = p.w[k]; t.dv = p.w[P + k]; t.dzt = p.w[2 * P + k];
+    t.dpu = p.w[3 * P + k]; t.dpv = p.w[4 * P + k]; t.dpz = p.w[5 * P + k];
   }
   int status = AW_ST_LIVE;
 
   for (int chk = 0; chk < p.nchk; ++chk) {
-    drift_angles<TAN>(t, p.a_open);  // opening drift of the block
+    const double px0 = t.pu, py0 = t.pv;
+    rotate_in<TAN>(t);                              // (x, y, z) -> (u, v, zeta)
+    drift_angles<TAN>(t, p.a_open, 2.0 * p.a_open);  // opening drift of the block
     resync<TAN, LEVEL>(t);           // pairs from the angles: the same values a new launch would start from
 
 #pragma unroll 1
@@ -226,45 +275,48 @@ __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS)
       for (int i = m; i > 0; --i) stages<S, TAN, LEVEL, 0>(t, p);
       if (rem > 0) resync<TAN, LEVEL>(t);
     }
-    drift_angles<TAN>(t, -p.a_open);  // last merged drift -> closing drift of the block
+    drift_angles<TAN>(t, -p.a_open, -2.0 * p.a_open);  // last merged drift -> closing drift of the block
+    rotate_out<TAN>(t, px0, py0);                      // (u, v, zeta) -> (x, y, z)
+    double &x = t.u, &y = t.v, &z = t.zt, &px = t.pu, &py = t.pv, &pz = t.pzt;
+    double &dx = t.du, &dy = t.dv, &dz = t.dzt, &dpx = t.dpu, &dpy = t.dpv;
 
     // ---- fused checkpoint (R4): (i) renormalise + log growth, (ii) energy error, (iii) wrap
     bool finite = true;
     if (TAN) {
-      double s2 = t.dx * t.dx;
-      s2 = fma(t.dy, t.dy, s2); s2 = fma(t.dz, t.dz, s2);
-      s2 = fma(t.dpx, t.dpx, s2); s2 = fma(t.dpy, t.dpy, s2); s2 = fma(t.dpz, t.dpz, s2);
+      double s2 = dx * dx;
+      s2 = fma(dy, dy, s2); s2 = fma(dz, dz, s2);
+      s2 = fma(dpx, dpx, s2); s2 = fma(dpy, dpy, s2); s2 = fma(t.dpz, t.dpz, s2);
       const double nu = sqrt(s2);
       const double inv = 1.0 / nu;
-      t.dx *= inv; t.dy *= inv; t.dz *= inv; t.dpx *= inv; t.dpy *= inv; t.dpz *= inv;
+      dx *= inv; dy *= inv; dz *= inv; dpx *= inv; dpy *= inv; t.dpz *= inv;
       const double logsum = p.acc[k] + log(nu);
       p.acc[k] = logsum;
       if (logsum > p.acc[P + k]) p.acc[P + k] = logsum;
-      finite = isfinite(t.dx) && isfinite(t.dy) && isfinite(t.dz) && isfinite(t.dpx) && isfinite(t.dpy) &&
+      finite = isfinite(dx) && isfinite(dy) && isfinite(dz) && isfinite(dpx) && isfinite(dpy) &&
                isfinite(t.dpz);
     }
-    const double dH = fabs(hamiltonian_dev(t.x, t.y, t.z, t.px, t.py, t.pz, p.eps) - p.acc[2 * P + k]);
+    const double dH = fabs(hamiltonian_dev(x, y, z, px, py, pz, p.eps) - p.acc[2 * P + k]);
     if (dH > p.acc[3 * P + k]) p.acc[3 * P + k] = dH;
     int tx, ty, tz;
-    t.x = wrap_angle(t.x, tx); t.y = wrap_angle(t.y, ty); t.z = wrap_angle(t.z, tz);
+    x = wrap_angle(x, tx); y = wrap_angle(y, ty); z = wrap_angle(z, tz);
     if (p.wind) {
       p.wind[k] += tx; p.wind[P + k] += ty; p.wind[2 * P + k] += tz;
     }
-    finite = finite && isfinite(t.x) && isfinite(t.y) && isfinite(t.z) && isfinite(t.px) && isfinite(t.py) &&
-             isfinite(t.pz);
+    finite = finite && isfinite(x) && isfinite(y) && isfinite(z) && isfinite(px) && isfinite(py) &&
+             isfinite(pz);
     if (!finite) { status = AW_ST_NONFINITE; break; }
     // survivor filter (R25): outside the launch rectangle at a checkpoint -> dropped, frozen here
-    if (p.survive && !(t.px >= p.surv[0] && t.px < p.surv[1] && t.py >= p.surv[2] && t.py < p.surv[3])) {
+    if (p.survive && !(px >= p.surv[0] && px < p.surv[1] && py >= p.surv[2] && py < p.surv[3])) {
       status = AW_ST_LEFT;
       break;
     }
   }
 
-  p.q[k] = t.x; p.q[P + k] = t.y; p.q[2 * P + k] = t.z;
-  p.q[3 * P + k] = t.px; p.q[4 * P + k] = t.py; p.q[5 * P + k] = t.pz;
+  p.q[k] = t.u; p.q[P + k] = t.v; p.q[2 * P + k] = t.zt;
+  p.q[3 * P + k] = t.pu; p.q[4 * P + k] = t.pv; p.q[5 * P + k] = t.pzt;
   if (TAN) {
-    p.w[k] = t.dx; p.w[P + k] = t.dy; p.w[2 * P + k] = t.dz;
-    p.w[3 * P + k] = t.dpx; p.w[4 * P + k] = t.dpy; p.w[5 * P + k] = t.dpz;
+    p.w[k] = t.du; p.w[P + k] = t.dv; p.w[2 * P + k] = t.dzt;
+    p.w[3 * P + k] = t.dpu; p.w[4 * P + k] = t.dpv; p.w[5 * P + k] = t.dpz;
   }
   if (status != AW_ST_LIVE) p.status[k] = (uint8_t)status;
 }
@@ -290,18 +342,19 @@ cudaError_t launch_level(const IntegrateParams &p, cudaStream_t st) {
 
 }  // namespace
 
-// Largest |d| each level may see on the x/y pairs (the 2z pair sees 2|d|) with both Taylor truncations
-// below 2^-60 ~ 8.7e-19 (they are systematic, so 300 of them still sum to < 3e-16):
-//   m of degree N truncates at |d|^(2N+2)/(2N+2)!, g at |d|^(2N+3)/(2N+3)!:
-//   N = 3: |d| <= 0.0208 (m), 0.0408 (g);  N = 4: 0.0708, 0.112;  N = 5: 0.165, 0.23.
-// level 1 = (3,3): 2|d| <= 0.0208;  level 2 = (3,4): |d| <= 0.0208;  level 3 = (4,4): 2|d| <= 0.0708;
-// level 4 = (4,5): |d| <= 0.0708;  beyond: level 0 (full sincos every stage).
+// Largest |d| = max_s |a_s| max|P| each level may see, with both Taylor truncations below 2^-60 ~ 8.7e-19 (they
+// are systematic, so 300 of them still sum to < 3e-16):
+//   m of degree N truncates at |t|^(2N+2)/(2N+2)!, g at |t|^(2N+3)/(2N+3)! for a rotation angle t:
+//   N = 3: |t| <= 0.0208 (m), 0.0408 (g);  N = 4: 0.0708, 0.112;  N = 5: 0.165, 0.23.
+// The u and v pairs rotate by up to sqrt(2) |d|, the 2z pair by up to 2 |d|:
+//   level 1 = (3,3): 2|d| <= 0.0208;  level 2 = (3,4): sqrt(2)|d| <= 0.0208;  level 3 = (4,4): 2|d| <= 0.0708;
+//   level 4 = (4,5): sqrt(2)|d| <= 0.0708;  beyond: level 0 (full sincos every stage).
 int trig_level_for(double d) {
   if (!(d == d)) return 0;
   if (d <= 0.0104) return 1;
-  if (d <= 0.0208) return 2;
+  if (d <= 0.0147) return 2;
   if (d <= 0.0354) return 3;
-  if (d <= 0.0708) return 4;
+  if (d <= 0.0500) return 4;
   return 0;
 }
 

@@ -26,18 +26,16 @@ struct IntegrateParams {
   int32_t level;   // trigonometry variant picked on the host from the largest drift angle (aw_integrate.cu)
   double a_open;   // a_1 (= a_{S+1}): angle drift that opens a block of `stride` steps; the block is closed by
                    // the angle drift -a_open, which takes the last merged drift back to the step boundary
-  double a2_loop[kMaxStages]; // 2 a_loop[s] (exact): drift of the angle 2z
+  double a2_loop[kMaxStages]; // 2 a_loop[s] (exact): tangent drift of dzeta = 2 dz with dpz
   double a_loop[kMaxStages];  // drift after kick s (s = 0..S-1): a_2 .. a_S, then a_{S+1} + a_1 (closing drift
                               // of one step merged with the opening drift of the next)
-  // Rotation of the running (sin, cos) pairs through the drift after kick s by the angle d = A p, A = a_loop[s]
-  // for the x and y pairs and 2 a_loop[s] for the 2z pair, as polynomials in z = p^2 (aw_integrate.cu):
+  // Rotation of the running (sin, cos) pairs through the drift after kick s by the angle d = A p, A = a_loop[s],
+  // p = pu, pv or pzeta, as polynomials in z = p^2 (aw_integrate.cu):
   //   sin d = p (G[0] + G[1] z + ...),  G[i] = (-1)^i A^(2i+1) / (2i+1)!      (G[0] = A exactly)
   //   cos d - 1 = z (M[0] + M[1] z + ...),  M[i] = (-1)^(i+1) A^(2i+2) / (2i+2)!
-  double gxy[kMaxStages][kTrigTerms + 1], mxy[kMaxStages][kTrigTerms];
-  double gz[kMaxStages][kTrigTerms + 1], mz[kMaxStages][kTrigTerms];
+  double grot[kMaxStages][kTrigTerms + 1], mrot[kMaxStages][kTrigTerms];
   double b1[kMaxStages];     // b_s
   double b2[kMaxStages];     // 2 b_s
-  double b4[kMaxStages];     // 4 b_s
   double eps;
   int32_t survive;  // survivor filter (R25): 1 = test (px, py) against surv[] at every checkpoint
   double surv[4];   // lo_x, hi_x, lo_y, hi_y (half-open)
@@ -86,6 +84,9 @@ cudaError_t launch_hamiltonian_probe(const double *q, int64_t n, int64_t pitch, 
                                      cudaStream_t st);
 cudaError_t launch_dfma_peak(int blocks, int threads, int chains, int64_t iters, double *sink,
                              cudaStream_t st);
+
+cudaError_t launch_dfma_shape(int blocks, int threads, int shape, int64_t iters, double *sink, const double *in,
+                              cudaStream_t st);
 
 void count_launch();
 

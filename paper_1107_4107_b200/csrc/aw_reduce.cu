@@ -182,7 +182,60 @@ __global__ void dfma_peak_kernel(int64_t iters, double *sink) {
   if (acc == 123.456) sink[0] = acc;  // never true in practice; keeps the chains alive
 }
 
+// fp64 issue rate by operand shape: 8 independent chains per thread, 32 instructions per loop trip.
+//   0: fma(v, u0, w0)    three registers, two of them shared by neighbouring instructions (reuse cache)
+//   1: fma(v, u_c, w_c)  three distinct registers, nothing shared with the neighbours
+//   2: fma(v, u_c, imm)  two registers + an immediate
+//   3: fma(v, v, w_c)    three register operands, two distinct
+//   4: v * u_c           DMUL, two registers
+//   5: fma(u_c, w_c', v) accumulate form, three distinct registers
+template <int SHAPE>
+__global__ void dfma_shape_kernel(int64_t iters, double *sink, const double *in) {
+  constexpr int CH = 8;
+  double v[CH], u[CH], w[CH];
+#pragma unroll
+  for (int c = 0; c < CH; ++c) {
+    v[c] = in[(threadIdx.x + c) & 127];
+    u[c] = in[(threadIdx.x + 32 + c) & 127];
+    w[c] = in[(threadIdx.x + 64 + c) & 127];
+  }
+#pragma unroll 1
+  for (int64_t i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+#pragma unroll
+      for (int c = 0; c < CH; ++c) {
+        if (SHAPE == 0) v[c] = fma(v[c], u[0], w[0]);
+        if (SHAPE == 1) v[c] = fma(v[c], u[c], w[c]);
+        if (SHAPE == 2) v[c] = fma(v[c], u[c], 1e-12);
+        if (SHAPE == 3) v[c] = fma(v[c], v[c], w[c]);
+        if (SHAPE == 4) v[c] = v[c] * u[c];
+        if (SHAPE == 5) v[c] = fma(u[c], w[(c + 1) % CH], v[c]);
+      }
+    }
+  }
+  double acc = 0.0;
+#pragma unroll
+  for (int c = 0; c < CH; ++c) acc += v[c];
+  if (acc == 123.456) sink[0] = acc;
+}
+
 }  // namespace
+
+cudaError_t launch_dfma_shape(int blocks, int threads, int shape, int64_t iters, double *sink, const double *in,
+                              cudaStream_t st) {
+  switch (shape) {
+    case 0: dfma_shape_kernel<0><<<blocks, threads, 0, st>>>(iters, sink, in); break;
+    case 1: dfma_shape_kernel<1><<<blocks, threads, 0, st>>>(iters, sink, in); break;
+    case 2: dfma_shape_kernel<2><<<blocks, threads, 0, st>>>(iters, sink, in); break;
+    case 3: dfma_shape_kernel<3><<<blocks, threads, 0, st>>>(iters, sink, in); break;
+    case 4: dfma_shape_kernel<4><<<blocks, threads, 0, st>>>(iters, sink, in); break;
+    case 5: dfma_shape_kernel<5><<<blocks, threads, 0, st>>>(iters, sink, in); break;
+    default: return cudaErrorInvalidValue;
+  }
+  count_launch();
+  return cudaGetLastError();
+}
 
 cudaError_t launch_indicator(const double *acc, const uint8_t *status, int64_t n, int64_t pitch, int kind,
                              double thr, double t, void *out, cudaStream_t st) {

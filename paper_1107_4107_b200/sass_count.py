@@ -43,12 +43,34 @@ def integrate_step_mix(order, tangent, level, lib=LIB):
         inner = [l for l in loops if not any(o != l and o[0] >= l[0] and o[1] <= l[1] for o in loops)]
         lo, hi = max(inner, key=lambda l: l[1] - l[0])      # the step loop is the longest innermost loop
         c = collections.Counter()
+        cycles, three, prev_reuse = 0, 0, {}
         for addr, t in ins:
-            if lo <= addr <= hi:
-                c[re.sub(r"^@!?U?P\d+\s+", "", t).split()[0].split(".")[0]] += 1
+            if not lo <= addr <= hi:
+                continue
+            t = re.sub(r"^@!?U?P\d+\s+", "", t)
+            op = t.split()[0]
+            c[op.split(".")[0]] += 1
+            if op.split(".")[0] not in ("DFMA", "DMUL", "DADD"):
+                continue
+            # issue-cycle model measured with aw_dfma_shape_probe (profiles/r1c_dfma_operand_shapes.md): an fp64
+            # instruction holds the pipe 2 cycles, 3 if it reads three distinct 64-bit registers none of which
+            # the previous fp64 instruction left in the operand-reuse cache (".reuse" in the same slot)
+            regs, cur = set(), {}
+            for slot, src in enumerate(x.strip() for x in t[len(op):].split(",")[1:]):
+                m = re.match(r"[-|]*R(\d+)", src)
+                if not m:
+                    continue
+                if prev_reuse.get(slot) != m.group(1):
+                    regs.add(m.group(1))
+                if ".reuse" in src:
+                    cur[slot] = m.group(1)
+            prev_reuse = cur
+            cycles += max(2, len(regs))
+            three += len(regs) >= 3
         fp = c["DFMA"] + c["DMUL"] + c["DADD"]
         mix = {"dfma": c["DFMA"], "dmul": c["DMUL"], "dadd": c["DADD"], "other": sum(c.values()) - fp,
-               "flops": 2 * c["DFMA"] + c["DMUL"] + c["DADD"]}
+               "flops": 2 * c["DFMA"] + c["DMUL"] + c["DADD"],
+               "issue_cycles": cycles, "three_register_fp64": three}
         _cache[key] = mix
         return mix
     raise KeyError(tag)
