@@ -268,10 +268,15 @@ def run_ours(args, cfg, order, tangent):
     achieved = kernel_rate * flops_per_step / 1e12
     sms = torch.cuda.get_device_properties(dev).multi_processor_count
     fp64_slots = sms * 64 * 1.965e9                                      # fp64 thread-instructions / s
+    # dram__bytes_read.sum + dram__bytes_write.sum of one 20 000-step launch of integrate_kernel<3,true,1> on the
+    # configs[3] grid, from the ncu --set full capture summarised in profiles/ (null for any other launch shape)
+    traffic, traffic_src = None, None
+    if (args.config, order, tangent, level) == (3, 4, True, 1) and steps_per_launch == 20000 and world == 1:
+        traffic, traffic_src = 628724992 + 525676288, "profiles/r1c_integrate_o4_tangent_ncu_full.md"
     roofline = {"bound": "alu",
                 "kernel": "integrate_kernel<%d,%s,%d>" % (3 if order == 4 else 7, str(tangent).lower(), level),
                 "achieved": achieved, "peak": FP64_PEAK_TFLOPS_NOMINAL, "unit": "TFLOP/s",
-                "frac": achieved / FP64_PEAK_TFLOPS_NOMINAL, "traffic": None,
+                "frac": achieved / FP64_PEAK_TFLOPS_NOMINAL, "traffic": traffic, "traffic_source": traffic_src,
                 "peak_source": "derived: 148 SM x 64 DFMA/clk/SM x 2 flop x 1.965 GHz (DESIGN.md §6.1); "
                                "MEASURED_PEAKS.json has no fp64 entry",
                 "flops_per_traj_step": flops_per_step, "flops_per_traj_step_nominal": flops_nominal,
