@@ -197,7 +197,9 @@ def run_ours(args, cfg, order, tangent):
     lo_y, hi_y = parallel.strip_bounds(cfg["lo"], cfg["hi"], world, rank)   # rank's strip of the image
     grid = aw.make_grid(gx, gy, cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"], cfg["cx"], cfg["cy"],
                         cfg["r"], 1, 0, lo_y=lo_y, hi_y=hi_y)
-    ens = aw.Ensemble(n, tangent=tangent, wind=True, order=order, device=dev)
+    dens_mode = cfg.get("density_mode", 0)          # 0: instantaneous actions; 1-3: the paper's averaged velocity
+    hist_lo, hist_hi = cfg.get("hist_lo", HIST_LO), cfg.get("hist_hi", HIST_HI)
+    ens = aw.Ensemble(n, tangent=tangent, wind=True, order=order, device=dev, ref=dens_mode != 0)
     image = torch.empty(n, dtype=torch.float64, device=dev)
     hist = torch.zeros((HIST_G, HIST_G), dtype=torch.int32, device=dev)
     dropped = torch.zeros(1, dtype=torch.int64, device=dev)
@@ -210,6 +212,8 @@ def run_ours(args, cfg, order, tangent):
         aw.aw_init_shell(ens, grid, cfg["E"], cfg["eps"], cfg["seed"])
         hist.zero_()
         dropped.zero_()
+        if dens_mode:
+            aw.aw_mark(ens)                          # X(t) of the averaging window
         if record:
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(stream)
@@ -218,7 +222,7 @@ def run_ours(args, cfg, order, tangent):
             e1.record(stream)
             integ_events.append((e0, e1))
         aw.aw_indicator(ens, kind, 0.0, out=image)
-        aw.aw_density(ens, hist, HIST_LO, HIST_HI, 0, dropped)
+        aw.aw_density(ens, hist, hist_lo, hist_hi, dens_mode, dropped)
         if world > 1:
             parallel.allreduce_hist(hist)
 
@@ -298,7 +302,9 @@ def run_ours(args, cfg, order, tangent):
             "config": {"workload": cfg["name"], "grid": [gx, gy], "trajectories_per_gpu": n,
                        "live_trajectories": live_all, "eps": cfg["eps"], "E": cfg["E"], "dt": cfg["dt"],
                        "steps_per_pass": horizon, "stride": cfg["stride"], "order": order,
-                       "tangent": tangent, "outputs": "FLI image fp64 + 1024x1024 uint32 density",
+                       "tangent": tangent,
+                       "outputs": ("FLI image fp64" if tangent else "max|dH| image fp64") + " + 1024x1024 uint32 density"
+                                  + (" of the projected averaged velocity (mode %d)" % dens_mode if dens_mode else ""),
                        "parallelism": "dp%d (one image strip per rank)" % world,
                        "l2": "state planes %.0f MB per pass > 126 MB L2 (no flush needed)"
                              % (n * (16 * 8 + 12 + 1) / 1e6)},
@@ -318,7 +324,7 @@ def run_ours(args, cfg, order, tangent):
             roofline["peak_probe_error"] = str(e)
 
     # e2e: host (pinned) state -> aw_map_host -> image + histogram on the host, copies inside the timing
-    if not args.no_e2e:
+    if not args.no_e2e and dens_mode == 0:          # aw_map_host bins the instantaneous actions (mode 0) only
         aw.aw_init_shell(ens, grid, cfg["E"], cfg["eps"], cfg["seed"])
         torch.cuda.synchronize()
         host_in = dict(q=ens.q.cpu().pin_memory(), acc=ens.acc.cpu().pin_memory(),

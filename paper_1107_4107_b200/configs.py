@@ -23,6 +23,18 @@ CONFIGS = {
     4: dict(name="cfg4_diffusion_2^20", gx=1024, gy=1024, lo=-1.0, hi=1.0, angle_mode=1, shape=1,
             cx=0.0, cy=0.0, r=1e-3, E=1.0, eps=1e-3, seed=0, order=4, dt=0.01, steps=10_000_000,
             stride=100, tangent=False, density_every=10_000),
+    # The paper's own workloads in its own units (eps = 1, T = 2 pi, h = 0.01 T, sixth-order scheme; P:55, P:85,
+    # P:89): initial conditions uniform on the sphere S x torus, averaging window Dt = 50 T = 5000 steps, density of
+    # the projected averaged velocity on the sphere (aw_mark + aw_density mode 3).  N = 2^22 stands in for the
+    # paper's N ~ 1e8; the figures themselves cannot be compared (not in the container).
+    5: dict(name="paper_fig2a_E400_sphere_velocity", gx=2048, gy=2048, lo=-1.0, hi=1.0, angle_mode=1, shape=3,
+            cx=0.0, cy=0.0, r=0.0, E=400.0, eps=1.0, seed=2011, order=6, dt=0.06283185307179587, steps=5_000,
+            stride=100, tangent=False, density_every=0, density_mode=3, hist_lo=-28.284271247461902,
+            hist_hi=28.284271247461902),
+    6: dict(name="paper_fig3a_E15_sphere_velocity", gx=2048, gy=2048, lo=-1.0, hi=1.0, angle_mode=1, shape=3,
+            cx=0.0, cy=0.0, r=0.0, E=15.0, eps=1.0, seed=2011, order=6, dt=0.06283185307179587, steps=5_000,
+            stride=100, tangent=False, density_every=0, density_mode=3, hist_lo=-5.477225575051661,
+            hist_hi=5.477225575051661),
 }
 
 HIST_G = 1024          # density histogram is HIST_G x HIST_G over [HIST_LO, HIST_HI]^2 (configs[4])

@@ -254,3 +254,117 @@ def test_mark_and_velocity_edge_cases(aw):
     assert int(hist.sum().item()) == 0 and int(dropped.item()) == 33
     assert bool(torch.isnan(aw.aw_indicator(e2, aw.AW_IND_VX)).all())
     assert bool((aw.aw_indicator(e2, aw.AW_IND_DP) == 0).all())
+
+
+# ------------------------------------------------------------------ full size, bench launch configurations
+
+def _sampled_full_size(aw, orc, cfg, steps, ref=False):
+    """aw_init_shell at the config's full size, `steps` steps on the GPU, and the oracle on a sample of
+    trajectories (a coarse lattice + 512 hashed pixels); returns (ens, oracle state, device copy, sample)."""
+    n = cfg["gx"] * cfg["gy"]
+    ens = aw.Ensemble(n, tangent=cfg["tangent"], wind=True, order=cfg["order"], ref=ref)
+    g = aw.make_grid(cfg["gx"], cfg["gy"], cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"], cfg["cx"],
+                     cfg["cy"], cfg["r"])
+    aw.aw_init_shell(ens, g, cfg["E"], cfg["eps"], cfg["seed"])
+    if ref:
+        aw.aw_mark(ens)
+    st = ensemble_to_oracle(ens, orc)
+    G = cfg["gx"]
+    rows = np.arange(0, G, max(1, G // 8))
+    lattice = (rows[:, None] * G + rows[None, :]).ravel()
+    hashed = np.array([orc.mix64(11, i) % n for i in range(512)], dtype=np.int64)
+    sample = np.unique(np.concatenate([lattice, hashed, [0, n - 1]]))
+    aw.aw_integrate(ens, n, steps, cfg["dt"], cfg["stride"])
+    for k in sample:
+        orc.integrate(st, steps, cfg["dt"], cfg["stride"], k0=int(k), k1=int(k) + 1, advance_clock=False)
+    st.t += steps * abs(cfg["dt"])
+    return ens, st, ensemble_to_oracle(ens, orc), sample
+
+
+@pytest.mark.parametrize("cfgk", [1, 2])
+def test_configs_1_2_full_grid_sampled_parity(aw, orc, cfgk):
+    """BASELINE configs[1] (512 x 512, eps = 1e-3, level 3) and configs[2] (1024 x 1024, eps = 1e-4, dt = 0.02,
+    seeded angles, level 4) at full size in the launch configuration bench.py would time; 1000 steps."""
+    cfg = aw.CONFIGS[cfgk]
+    ens, st, got, sample = _sampled_full_size(aw, orc, cfg, 1000)
+    assert aw.aw_trig_level(ens, cfg["dt"]) == (3 if cfgk == 1 else 4)
+    assert np.array_equal(got.status[sample], st.status[sample])
+    live = st.status[sample] == 1
+    thr = math.log(1000 * cfg["dt"]) + 3.0
+    regular = live & (st.acc[1, sample] <= thr)
+    assert regular.sum() > 0.9 * live.sum()
+    err = state_rel_err(got.q[:, sample], got.wind[:, sample], st.q[:, sample], st.wind[:, sample], regular)
+    assert err.max() <= 1e-10, err.max()
+    assert np.max(np.abs(got.acc[1, sample][regular] - st.acc[1, sample][regular])) <= 1e-5
+    # class image: pixel for pixel outside the 1 % band
+    band = np.abs(st.acc[1, sample] - thr) < 0.01 * thr
+    cls = aw.aw_indicator(ens, aw.AW_IND_CLASS, thr).cpu().numpy()[sample]
+    ref = np.where(live, (st.acc[1, sample] > thr).astype(np.uint8), 255)
+    assert np.array_equal(cls[~band], ref[~band])
+    # at full size: every live trajectory on the shell layer (P:51) with a bounded energy error
+    n = ens.n
+    livef = got.status == 1
+    dH = got.acc[3, :n][livef]
+    assert dH.max() < 1e-9
+    P2 = np.sum(got.q[3:, :n][:, livef] ** 2, axis=0)
+    assert np.all(np.abs(P2 - 2.0) <= 4 * cfg["eps"] + 2 * dH.max())
+
+
+def test_config4_full_cloud_parity_and_density(aw, orc):
+    """BASELINE configs[4] at full size: 2^20 trajectories in a disk of radius 1e-3 at the resonance crossing
+    (0, 0, sqrt 2); 1000 steps on the GPU, sampled state parity, and the 1024 x 1024 histogram bit-exact against
+    the oracle's binning of the device states at three binning events (the first with all points in <= 4 bins)."""
+    cfg = aw.CONFIGS[4]
+    n = cfg["gx"] * cfg["gy"]
+    assert n == 1 << 20
+    ens = aw.Ensemble(n, tangent=False, wind=True, order=4)
+    g = aw.make_grid(cfg["gx"], cfg["gy"], cfg["lo"], cfg["hi"], 1, cfg["shape"], cfg["cx"], cfg["cy"], cfg["r"])
+    aw.aw_init_shell(ens, g, cfg["E"], cfg["eps"], cfg["seed"])
+    hist = torch.zeros((1024, 1024), dtype=torch.int32, device="cuda")
+    dropped = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ref = np.zeros((1024, 1024), dtype=np.uint32)
+    d = np.zeros(1, dtype=np.uint64)
+    st0 = ensemble_to_oracle(ens, orc)
+    sample = np.array([orc.mix64(4, i) % n for i in range(256)], dtype=np.int64)
+    for event in range(3):
+        aw.aw_density(ens, hist, -1.0, 1.0, 0, dropped)
+        orc.density(ensemble_to_oracle(ens, orc), ref, -1.0, 1.0, d)
+        h = hist.cpu().numpy().view(np.uint32)
+        assert np.array_equal(h, ref) and int(dropped.item()) == int(d[0]) == 0
+        assert h.sum() == (event + 1) * n
+        if event == 0:
+            assert (h > 0).sum() <= 4
+        if event < 2:
+            aw.aw_integrate(ens, n, 500, cfg["dt"], cfg["stride"])
+    for k in sample:
+        orc.integrate(st0, 1000, cfg["dt"], cfg["stride"], k0=int(k), k1=int(k) + 1, advance_clock=False)
+    got = ensemble_to_oracle(ens, orc)
+    err = state_rel_err(got.q[:, sample], got.wind[:, sample], st0.q[:, sample], st0.wind[:, sample],
+                        np.ones(len(sample), bool))
+    assert err.max() <= 1e-10, err.max()
+    tol = 64 * 2.0 ** -52 + 0.01 * st0.acc[3, sample]
+    assert np.all(np.abs(got.acc[3, sample] - st0.acc[3, sample]) <= tol)
+
+
+def test_paper_workload_full_size_sampled_parity(aw, orc):
+    """configs 6 (the paper's Fig. 3a workload in its own units: E = 15, eps = 1, sixth order, h = 0.01 T, 2^22
+    initial conditions uniform on S x torus) in the launch configuration bench.py --config 6 times: state parity
+    on sampled trajectories after 100 steps, then the sphere density bit-exact on the device states."""
+    cfg = aw.CONFIGS[6]
+    ens, st, got, sample = _sampled_full_size(aw, orc, cfg, 100, ref=True)
+    assert np.all(got.status == 1)
+    err = state_rel_err(got.q[:, sample], got.wind[:, sample], st.q[:, sample], st.wind[:, sample],
+                        np.ones(len(sample), bool))
+    assert err.max() <= 1e-10, err.max()
+    hist = torch.zeros((1024, 1024), dtype=torch.int32, device="cuda")
+    dropped = torch.zeros(1, dtype=torch.int64, device="cuda")
+    aw.aw_density(ens, hist, cfg["hist_lo"], cfg["hist_hi"], cfg["density_mode"], dropped)
+    ref = np.zeros((1024, 1024), dtype=np.uint32)
+    d = orc.density_velocity(got, ref, cfg["hist_lo"], cfg["hist_hi"], cfg["density_mode"])
+    h = hist.cpu().numpy().view(np.uint32)
+    assert np.array_equal(h, ref) and int(dropped.item()) == int(d[0])
+    assert int(h.sum()) + int(d[0]) == ens.n
+    # the projected points fill the disk |Vhat_xy| <= sqrt(2E) and nothing outside it
+    yy, xx = np.mgrid[0:1024, 0:1024]
+    r2 = ((xx + 0.5) / 512 - 1) ** 2 + ((yy + 0.5) / 512 - 1) ** 2
+    assert h[r2 > 1.01].sum() == 0 and (h[r2 < 0.9] > 0).mean() > 0.85
