@@ -217,14 +217,14 @@ __device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2) {
     sincos(t.v, t.sv, t.cv);
     sincos(t.zt, t.s2, t.c2);
   }
-  const double F = fma(b1, t.c2, b1);  // b (1 + cos zeta)
-  const double G2 = b2 * t.s2;         // 2 b sin zeta
-  const double w = t.cu + t.cv;        // 2 cos x cos y
+  const double F = fma(b1, t.c2, b1);          // b (1 + cos zeta)
+  const double G = TAN ? b1 * t.s2 : 0.0;      // b sin zeta
+  const double G2 = TAN ? G + G : b2 * t.s2;   // 2 b sin zeta (one stage constant fewer in the tangent kernels)
+  const double w = t.cu + t.cv;                // 2 cos x cos y
   t.pu = fma(t.su, F, t.pu);
   t.pv = fma(t.sv, F, t.pv);
   t.pzt = fma(w, G2, t.pzt);
   if (TAN) {
-    const double G = b1 * t.s2;  // b sin zeta
     const double a1 = F * t.cu, a2 = F * t.cv, k1 = G * t.su, k2 = G * t.sv;
     const double e5 = w * (b1 * t.c2);  // b (cos u + cos v) cos zeta
     t.dpu = fma(a1, t.du, t.dpu); t.dpv = fma(a2, t.dv, t.dpv); t.dpz = fma(e5, t.dzt, t.dpz);
@@ -237,7 +237,8 @@ __device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2) {
 template <int S, bool TAN, int LEVEL, int s>
 __device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p) {
   if constexpr (s < S) {
-    kick<TAN, LEVEL>(t, p.b1[s], p.b2[s]);
+    constexpr int bs = s < S - 1 - s ? s : S - 1 - s;  // palindromic weights: b_s == b_{S-1-s}
+    kick<TAN, LEVEL>(t, p.b1[bs], p.b2[bs]);
     drift<S, TAN, LEVEL, s>(t, p);
     stages<S, TAN, LEVEL, s + 1>(t, p);
   }

@@ -368,3 +368,52 @@ def test_paper_workload_full_size_sampled_parity(aw, orc):
     yy, xx = np.mgrid[0:1024, 0:1024]
     r2 = ((xx + 0.5) / 512 - 1) ** 2 + ((yy + 0.5) / 512 - 1) ** 2
     assert h[r2 > 1.01].sum() == 0 and (h[r2 < 0.9] > 0).mean() > 0.85
+
+
+@pytest.mark.parametrize("cfgk,nsample", [(1, 32), (3, 32), (2, 16)])
+def test_full_horizon_indicator_map_parity(aw, orc, cfgk, nsample):
+    """BASELINE configs[1..3] at full size over their FULL horizon (1e5 / 2e5 / 1e6 steps, the run bench.py times
+    for configs[3]) against the oracle on a fixed nsample x nsample sub-lattice of pixels (north_star: indicator
+    maps agree pixel for pixel on the regular/chaotic classification except within 1 % of the threshold; FLI
+    values agree to 1e-5 where FLI < 10 and 1e-2 where 10 <= FLI < 20)."""
+    cfg = aw.CONFIGS[cfgk]
+    G = cfg["gx"]
+    n = G * G
+    ens = aw.Ensemble(n, tangent=True, wind=True, order=cfg["order"])
+    g = aw.make_grid(G, G, cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"], cfg["cx"], cfg["cy"], cfg["r"])
+    aw.aw_init_shell(ens, g, cfg["E"], cfg["eps"], cfg["seed"])
+    rows = (np.arange(nsample) * (G // nsample) + G // (2 * nsample))
+    sample = (rows[:, None] * G + rows[None, :]).ravel()
+    full = ensemble_to_oracle(ens, orc)
+    sub = orc.State(len(sample), tangent=True, wind=True)            # the sampled pixels as a small ensemble
+    m = len(sample)
+    sub.q[:, :m], sub.w[:, :m], sub.acc[:, :m] = full.q[:, sample], full.w[:, sample], full.acc[:, sample]
+    sub.wind[:, :m], sub.status[:] = full.wind[:, sample], full.status[sample]
+    sub.E, sub.eps, sub.order = full.E, full.eps, full.order
+    aw.aw_integrate(ens, n, cfg["steps"], cfg["dt"], cfg["stride"])
+    from util import oracle_integrate_mt
+    oracle_integrate_mt(orc, sub, cfg["steps"], cfg["dt"], cfg["stride"])
+    torch.cuda.synchronize()
+    t_end = cfg["steps"] * cfg["dt"]
+    assert abs(ens.t - t_end) < 1e-6 * t_end and ens.step == cfg["steps"]
+    thr = math.log(t_end) + 3.0
+    fli = aw.aw_indicator(ens, aw.AW_IND_FLI).cpu().numpy()[sample]
+    cls = aw.aw_indicator(ens, aw.AW_IND_CLASS, thr).cpu().numpy()[sample]
+    status = ens.status[:n].cpu().numpy()[sample]
+    assert np.array_equal(status, sub.status)
+    live = sub.status == 1
+    ref = sub.acc[1, :m]
+    band = np.abs(ref - thr) < 0.01 * thr
+    ref_cls = np.where(live, (ref > thr).astype(np.uint8), 255)
+    mism = (cls != ref_cls) & ~band
+    print("config %d: %d sampled pixels, %d chaotic, %d inside the 1%% band, %d mismatches outside it"
+          % (cfgk, m, int((ref_cls == 1).sum()), int((band & live).sum()), int(mism.sum())))
+    assert mism.sum() == 0
+    lo10 = live & (ref < 10)
+    mid = live & (ref >= 10) & (ref < 20)
+    assert np.max(np.abs(fli[lo10] - ref[lo10])) <= 1e-5
+    if mid.any():
+        assert np.max(np.abs(fli[mid] - ref[mid])) <= 1e-2
+    # energy: bounded, no secular growth (P:55) on every live pixel of the full image
+    dH = aw.aw_indicator(ens, aw.AW_IND_DH).cpu().numpy()
+    assert np.nanmax(dH) < 1e-8
