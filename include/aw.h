@@ -155,7 +155,7 @@ AW_API int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps,
  * max_s |a_s| sqrt(2(E + 2|eps|)) so the truncation stays below 2^-60; aw_trig_level reports it), and
  * recomputes them from the angles with the device sincos at every checkpoint and at least every 128
  * steps.  s->E must therefore bound the energy of an uploaded state.  If the drift angle can exceed
- * 0.05 rad, or with s->trig == 1, the device sincos is evaluated at every stage instead (level 0).
+ * 0.357 rad, or with s->trig == 1, the device sincos is evaluated at every stage instead (level 0).
  * The work is split into kernel launches of at most AW_MAX_STEPS_PER_LAUNCH steps (a multiple of
  * stride); the result does not depend on the split. */
 #define AW_MAX_STEPS_PER_LAUNCH 20000
@@ -201,7 +201,8 @@ AW_API int aw_density(const aw_state *s, uint32_t *hist_dev, int32_t gx, int32_t
  * four order conditions in extended precision. */
 AW_API int aw_stage_constants(int order, double dt, double eps, double *a_host, double *b_host);
 /* Trigonometry level aw_integrate would use for this state and dt: 0 = device sincos at every stage,
- * 1..4 = running pairs with Taylor degrees (x+y / x-y pairs, 2z pair) = (3,3), (3,4), (4,4), (4,5); or a
+ * 1..7 = running pairs with Taylor degrees (x+y / x-y pairs, 2z pair) = (3,3), (3,4), (4,4), (4,5), (5,6),
+ * (6,7), (7,8); or a
  * negative aw_status.  Pure host arithmetic. */
 AW_API int aw_trig_level(const aw_state *s, double dt);
 /* The common tangent vector of tangent_mode 0: unit vector from u(seed, 2^63-1, 5..10) (R12). */

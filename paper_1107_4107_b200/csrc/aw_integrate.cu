@@ -76,9 +76,11 @@ __device__ __forceinline__ void small_sincos(double p, const double (&G)[kTrigTe
 // registers (a DFMA takes one constant-bank operand at most).  N + (N-1) FMA, 3 DMUL, plus d = A p outside.
 template <int N>
 __device__ __forceinline__ void small_sincos_angle(double d, double &g, double &m) {
-  constexpr double Sc[5] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0, -1.0 / 39916800.0};
-  constexpr double Cc[5] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0, -1.0 / 3628800.0};
-  static_assert(N >= 1 && N <= 5, "degree");
+  constexpr double Sc[8] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0, -1.0 / 39916800.0,
+                            1.0 / 6227020800.0, -1.0 / 1307674368000.0, 1.0 / 355687428096000.0};
+  constexpr double Cc[8] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0, -1.0 / 3628800.0,
+                            1.0 / 479001600.0, -1.0 / 87178291200.0, 1.0 / 20922789888000.0};
+  static_assert(N >= 1 && N <= 8, "degree");
   const double z = d * d;
   double pg = Sc[N - 1], pm = Cc[N - 1];
 #pragma unroll
@@ -107,6 +109,9 @@ template <> struct Deg<1> { static constexpr int uv = 3, z = 3; };
 template <> struct Deg<2> { static constexpr int uv = 3, z = 4; };
 template <> struct Deg<3> { static constexpr int uv = 4, z = 4; };
 template <> struct Deg<4> { static constexpr int uv = 4, z = 5; };
+template <> struct Deg<5> { static constexpr int uv = 5, z = 6; };
+template <> struct Deg<6> { static constexpr int uv = 6, z = 7; };
+template <> struct Deg<7> { static constexpr int uv = 7, z = 8; };
 
 // Everything a thread carries between stages.  Inside a block of `stride` steps the state is held in the
 // rotated and scaled variables
@@ -217,14 +222,14 @@ __device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2) {
     sincos(t.v, t.sv, t.cv);
     sincos(t.zt, t.s2, t.c2);
   }
-  const double F = fma(b1, t.c2, b1);          // b (1 + cos zeta)
-  const double G = TAN ? b1 * t.s2 : 0.0;      // b sin zeta
-  const double G2 = TAN ? G + G : b2 * t.s2;   // 2 b sin zeta (one stage constant fewer in the tangent kernels)
-  const double w = t.cu + t.cv;                // 2 cos x cos y
+  const double F = fma(b1, t.c2, b1);  // b (1 + cos zeta)
+  const double G2 = b2 * t.s2;         // 2 b sin zeta
+  const double w = t.cu + t.cv;        // 2 cos x cos y
   t.pu = fma(t.su, F, t.pu);
   t.pv = fma(t.sv, F, t.pv);
   t.pzt = fma(w, G2, t.pzt);
   if (TAN) {
+    const double G = b1 * t.s2;  // b sin zeta
     const double a1 = F * t.cu, a2 = F * t.cv, k1 = G * t.su, k2 = G * t.sv;
     const double e5 = w * (b1 * t.c2);  // b (cos u + cos v) cos zeta
     t.dpu = fma(a1, t.du, t.dpu); t.dpv = fma(a2, t.dv, t.dpv); t.dpz = fma(e5, t.dzt, t.dpz);
@@ -237,8 +242,7 @@ __device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2) {
 template <int S, bool TAN, int LEVEL, int s>
 __device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p) {
   if constexpr (s < S) {
-    constexpr int bs = s < S - 1 - s ? s : S - 1 - s;  // palindromic weights: b_s == b_{S-1-s}
-    kick<TAN, LEVEL>(t, p.b1[bs], p.b2[bs]);
+    kick<TAN, LEVEL>(t, p.b1[s], p.b2[s]);
     drift<S, TAN, LEVEL, s>(t, p);
     stages<S, TAN, LEVEL, s + 1>(t, p);
   }
@@ -337,6 +341,9 @@ cudaError_t launch_level(const IntegrateParams &p, cudaStream_t st) {
     case 2: return launch_one<S, TAN, 2>(p, st);
     case 3: return launch_one<S, TAN, 3>(p, st);
     case 4: return launch_one<S, TAN, 4>(p, st);
+    case 5: return launch_one<S, TAN, 5>(p, st);
+    case 6: return launch_one<S, TAN, 6>(p, st);
+    case 7: return launch_one<S, TAN, 7>(p, st);
     default: return launch_one<S, TAN, 0>(p, st);
   }
 }
@@ -345,17 +352,22 @@ cudaError_t launch_level(const IntegrateParams &p, cudaStream_t st) {
 
 // Largest |d| = max_s |a_s| max|P| each level may see, with both Taylor truncations below 2^-60 ~ 8.7e-19 (they
 // are systematic, so 300 of them still sum to < 3e-16):
-//   m of degree N truncates at |t|^(2N+2)/(2N+2)!, g at |t|^(2N+3)/(2N+3)! for a rotation angle t:
-//   N = 3: |t| <= 0.0208 (m), 0.0408 (g);  N = 4: 0.0708, 0.112;  N = 5: 0.165, 0.23.
+//   m of degree N truncates at |t|^(2N+2)/(2N+2)!, g at |t|^(2N+3)/(2N+3)! for a rotation angle t; the m bound
+//   is the tighter one:  N = 3: |t| <= 0.0208;  4: 0.0708;  5: 0.165;  6: 0.310;  7: 0.505;  8: 0.750.
 // The u and v pairs rotate by up to sqrt(2) |d|, the 2z pair by up to 2 |d|:
-//   level 1 = (3,3): 2|d| <= 0.0208;  level 2 = (3,4): sqrt(2)|d| <= 0.0208;  level 3 = (4,4): 2|d| <= 0.0708;
-//   level 4 = (4,5): sqrt(2)|d| <= 0.0708;  beyond: level 0 (full sincos every stage).
+//   level 1 = (3,3): 2|d| <= 0.0208;       level 2 = (3,4): sqrt(2)|d| <= 0.0208;   level 3 = (4,4): 2|d| <= 0.0708;
+//   level 4 = (4,5): sqrt(2)|d| <= 0.0708;  level 5 = (5,6): sqrt(2)|d| <= 0.165;    level 6 = (6,7): sqrt(2)|d| <= 0.310;
+//   level 7 = (7,8): sqrt(2)|d| <= 0.505 (and 2|d| <= 0.750);  beyond: level 0 (full sincos every stage), which is
+//   also cheaper from there on: a degree-(8,9) rotation costs more fp64 instructions than the sincos it replaces.
 int trig_level_for(double d) {
   if (!(d == d)) return 0;
   if (d <= 0.0104) return 1;
   if (d <= 0.0147) return 2;
   if (d <= 0.0354) return 3;
   if (d <= 0.0500) return 4;
+  if (d <= 0.1166) return 5;
+  if (d <= 0.2192) return 6;
+  if (d <= 0.3570) return 7;
   return 0;
 }
 

@@ -8,7 +8,7 @@
 namespace aw {
 
 constexpr int kMaxStages = 7;
-constexpr int kTrigTerms = 5;  // largest Taylor degree N of the drift rotations (level 4, 2z pair)
+constexpr int kTrigTerms = 8;  // largest Taylor degree N of the drift rotations (level 7, 2z pair)
 
 // Kernel parameters of the integrator; lives in the constant bank (__grid_constant__), so the stage
 // constants are constant-bank operands of the DFMA instructions and cost no registers.
