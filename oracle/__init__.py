@@ -83,6 +83,7 @@ def lib():
                                            C.c_double, C.c_int, _u32p, C.c_int32, C.c_int32, C.c_double,
                                            C.c_double, _u64p]
         L.awo_delta_p.argtypes = [C.c_int64, C.c_int64, _dp, _dp, _u8p, _dp]
+        L.awo_energy_stats.argtypes = [C.c_int64, C.c_int64, _dp, _dp, _u8p, C.c_double, _dp, _dp]
         _lib = L
     return _lib
 
@@ -286,3 +287,12 @@ def delta_p(state):
                            _p(state.status, _u8p), _p(out, _dp))
     assert rc == 0, rc
     return out
+
+
+def energy_stats(state):
+    """(stats[8], signed dH image[n]) — the energy-drift statistics of BASELINE configs[2] (R29)."""
+    out, img = np.zeros(8), np.zeros(state.n)
+    rc = lib().awo_energy_stats(state.n, state.pitch, _p(state.q, _dp), _p(state.acc, _dp),
+                                _p(state.status, _u8p), state.eps, _p(out, _dp), _p(img, _dp))
+    assert rc == 0, rc
+    return out, img

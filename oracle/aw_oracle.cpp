@@ -521,4 +521,40 @@ int awo_delta_p(int64_t n, int64_t pitch, const double *q, const double *qref, c
   return 0;
 }
 
+// "Energy-drift statistics" of BJ:configs[2] (R29): over the live trajectories, from the checkpointed maximum
+// dH_max = max_t |H(t) - H0| (acc plane 3) and the signed error of the CURRENT state, H(X, P) - H0:
+//   out[0] live count   out[1] max dH_max   out[2] mean dH_max   out[3] rms dH_max
+//   out[4] mean signed  out[5] rms signed   out[6] index of the trajectory with the largest dH_max (first one)
+//   out[7] max |signed|
+// A symplectic scheme shows no secular growth: the signed mean stays at the rounding level and
+// dH_max does not grow with t.  Plain left-to-right sums.  signed_out (may be NULL): the signed image, NaN
+// where the trajectory is not live.
+int awo_energy_stats(int64_t n, int64_t pitch, const double *q, const double *acc, const uint8_t *status,
+                     double eps, double *out, double *signed_out) {
+  if (!q || !acc || !status || !out) return -1;
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+  double cnt = 0.0, mx = 0.0, sum = 0.0, sq = 0.0, ssum = 0.0, ssq = 0.0, smax = 0.0, worst = -1.0;
+  for (int64_t k = 0; k < n; ++k) {
+    if (status[k] != 1) { if (signed_out) signed_out[k] = nan; continue; }
+    double st[6];
+    for (int c = 0; c < 6; ++c) st[c] = q[c * pitch + k];
+    const double sd = Hamiltonian(st, eps) - acc[2 * pitch + k];
+    const double d = acc[3 * pitch + k];
+    if (signed_out) signed_out[k] = sd;
+    cnt += 1.0;
+    if (d > mx || worst < 0.0) { mx = d; worst = (double)k; }
+    sum += d;
+    sq += d * d;
+    ssum += sd;
+    ssq += sd * sd;
+    if (std::fabs(sd) > smax) smax = std::fabs(sd);
+  }
+  out[0] = cnt; out[1] = mx; out[6] = worst; out[7] = smax;
+  out[2] = cnt > 0.0 ? sum / cnt : nan;
+  out[3] = cnt > 0.0 ? std::sqrt(sq / cnt) : nan;
+  out[4] = cnt > 0.0 ? ssum / cnt : nan;
+  out[5] = cnt > 0.0 ? std::sqrt(ssq / cnt) : nan;
+  return 0;
+}
+
 }  // extern "C"

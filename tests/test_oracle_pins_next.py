@@ -282,3 +282,55 @@ def test_P22_sphere_initial_conditions(orc):
     st2 = orc.State(n, tangent=False, wind=True)
     orc.init_shell(st2, orc.make_grid(256, 256, angle_mode=1, shape=3, pz_sign=-1), 1.0, 3e-2, 12345)
     assert np.array_equal(st2.q[5, :n], -st.q[5, :n]) and np.array_equal(st2.q[:5, :n], st.q[:5, :n])
+
+
+# ------------------------------------------------------------------ P23: energy-drift statistics (configs[2])
+
+def test_P23_energy_drift_statistics(orc):
+    """max / mean / rms of dH_max and mean / rms of the signed final error H(t) - H0 over the live trajectories:
+    (i) against numpy on the images (test-side arithmetic, mpmath H on a few pixels); (ii) eps = 0: every entry
+    is at the rounding level; (iii) P:55 "no secular growth": doubling the horizon leaves max dH_max within a
+    factor 1.5 and the signed mean stays far below the rms; (iv) order 6 beats order 4 by > 100 at dt = 0.02."""
+    import mpmath as mp
+    mp.mp.dps = 30
+    E, eps = 1.0, 1e-2
+    n = 40 * 30
+    st = orc.State(n, tangent=False, wind=True)
+    orc.init_shell(st, orc.make_grid(40, 30, -1.04, 1.04, angle_mode=1), E, eps, 21)
+    orc.integrate(st, 2000, 0.02, 100)
+    out, img = orc.energy_stats(st)
+    live = st.status == 1
+    assert 0 < (~live).sum() < n and np.all(np.isnan(img[~live])) and not np.any(np.isnan(img[live]))
+    d = st.acc[3, :n][live]
+    assert out[0] == live.sum() and out[1] == d.max()
+    assert abs(out[2] - d.mean()) < 1e-12 * d.mean() and abs(out[3] - math.sqrt((d * d).mean())) < 1e-12 * out[3]
+    assert np.nonzero(live)[0][np.argmax(d)] == int(out[6])
+    sd = img[live]
+    assert abs(out[4] - sd.mean()) < 1e-18 + 1e-9 * abs(sd).max() and abs(out[5] - math.sqrt((sd * sd).mean())) < 1e-12 * out[5]
+    assert out[7] == np.abs(sd).max() and out[7] <= out[1] * (1 + 1e-9) + 1e-15   # the final state is one sample
+    for k in np.nonzero(live)[0][:20]:
+        x, y, z, px, py, pz = (mp.mpf(float(v)) for v in st.q[:, k])
+        H = (px * px + py * py + pz * pz) / 2 + mp.mpf(eps) * mp.cos(x) * mp.cos(y) * (1 + mp.cos(2 * z))
+        assert abs(float(H - mp.mpf(float(st.acc[2, k]))) - img[k]) < 4e-16
+    # (iii) no secular growth
+    max1, mean_signed1 = out[1], out[4]
+    orc.integrate(st, 2000, 0.02, 100)
+    out2, _ = orc.energy_stats(st)
+    assert out2[1] < 1.5 * max1
+    assert abs(out2[4]) < 0.5 * out2[5]
+    # (iv) order
+    s6 = orc.State(n, tangent=False, wind=True)
+    orc.init_shell(s6, orc.make_grid(40, 30, -1.04, 1.04, angle_mode=1), E, eps, 21)
+    s6.order = 6
+    orc.integrate(s6, 2000, 0.02, 100)
+    assert orc.energy_stats(s6)[0][1] < max1 / 100
+    # (ii) eps = 0
+    s0 = orc.State(n, tangent=False, wind=True)
+    orc.init_shell(s0, orc.make_grid(40, 30, -0.9, 0.9, angle_mode=1), E, 0.0, 21)
+    orc.integrate(s0, 1000, 0.02, 100)
+    o0, i0 = orc.energy_stats(s0)
+    assert o0[0] == n and o0[1] == 0.0 and o0[7] == 0.0 and np.all(i0 == 0.0)
+    # empty ensemble: count 0, NaN means
+    e = orc.State(4, tangent=False, wind=True)
+    oe, _ = orc.energy_stats(e)
+    assert oe[0] == 0 and np.isnan(oe[2]) and oe[6] == -1
