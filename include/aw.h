@@ -53,7 +53,7 @@ typedef enum {
 
 /* indicator kinds for aw_indicator (R13, R14; DP: P:37; VX..VZ: P:67 + fn. 26) */
 enum { AW_IND_FLI = 0, AW_IND_FTLE = 1, AW_IND_DH = 2, AW_IND_CLASS = 3,
-       AW_IND_DP = 4, AW_IND_VX = 5, AW_IND_VY = 6, AW_IND_VZ = 7 };
+       AW_IND_DP = 4, AW_IND_VX = 5, AW_IND_VY = 6, AW_IND_VZ = 7, AW_IND_DHS = 8 };
 /* aw_density modes: instantaneous actions (BASELINE) or the paper's projected averaged velocity (R19, R26) */
 enum { AW_DENS_ACTION = 0, AW_DENS_VEL_UPPER = 1, AW_DENS_VEL_LOWER = 2, AW_DENS_VEL_BOTH = 3 };
 /* aw_grid.shape */
@@ -175,8 +175,19 @@ AW_API int aw_mark(aw_state *s);
  * §8(f): AW_IND_DP: |P - Pref| (three rounded squares summed left to right, IEEE sqrt).
  * AW_IND_VX / VY / VZ: component of the projected averaged velocity Vhat (see aw_density), NaN where
  * the trajectory is not live or |V| = 0.  These need s->qref (AW_ESTATE if NULL); VX..VZ also need
- * s->t > s->tref. */
+ * s->t > s->tref.
+ * AW_IND_DHS: the signed energy error of the CURRENT state, H(X,P) - H0, by the routine the checkpoint uses
+ * (BASELINE configs[2] "energy-drift statistics"; R29). */
 AW_API int aw_indicator(const aw_state *s, int kind, double thr, void *out_dev);
+
+/* Energy-drift statistics over the live trajectories (BASELINE configs[2]; R29; "no secular growth"):
+ * out_dev[0] live count, [1] max dH_max, [2] mean dH_max, [3] rms dH_max, [4] mean and [5] rms of the signed
+ * error H(X,P) - H0 of the current state, [6] index of the first trajectory attaining max dH_max (-1 if none),
+ * [7] max |signed error|; means are NaN for an empty ensemble.  out_dev: 8 doubles (device); scratch_dev: device,
+ * aw_energy_stats_scratch_bytes(n) bytes, 16-byte aligned.  Two kernels, deterministic (fixed reduction order,
+ * no floating-point atomics): the same state gives the same bits on every run. */
+AW_API size_t aw_energy_stats_scratch_bytes(int64_t n);
+AW_API int aw_energy_stats(const aw_state *s, void *scratch_dev, double *out_dev);
 
 /* §8(a) a6 — visited-cell density over the first two actions (R19, R20).  For each live
  * trajectory ix = floor((px - lo) * (gx/(hi - lo))), iy likewise with gy; inside -> hist[iy*gx + ix]

@@ -14,7 +14,7 @@ _LIBPATH = os.path.join(_HERE, "libaw.so")
 
 AW_OK, AW_EINVAL, AW_ECUDA, AW_ERANGE, AW_ESTATE = 0, -1, -2, -3, -4
 AW_IND_FLI, AW_IND_FTLE, AW_IND_DH, AW_IND_CLASS = 0, 1, 2, 3
-AW_IND_DP, AW_IND_VX, AW_IND_VY, AW_IND_VZ = 4, 5, 6, 7
+AW_IND_DP, AW_IND_VX, AW_IND_VY, AW_IND_VZ, AW_IND_DHS = 4, 5, 6, 7, 8
 AW_DENS_ACTION, AW_DENS_VEL_UPPER, AW_DENS_VEL_LOWER, AW_DENS_VEL_BOTH = 0, 1, 2, 3
 AW_SHAPE_GRID, AW_SHAPE_DISK, AW_SHAPE_GAUSS, AW_SHAPE_SPHERE = 0, 1, 2, 3
 AW_ST_OFFSHELL, AW_ST_LIVE, AW_ST_NONFINITE, AW_ST_LEFT = 0, 1, 2, 3
@@ -87,6 +87,9 @@ def lib():
         L.aw_init_shell.argtypes = [C.POINTER(AwState), C.POINTER(Grid), dbl, dbl, u64]
         L.aw_integrate.argtypes = [C.POINTER(AwState), i64, i64, dbl, i64]
         L.aw_mark.argtypes = [C.POINTER(AwState)]
+        L.aw_energy_stats_scratch_bytes.restype = C.c_size_t
+        L.aw_energy_stats_scratch_bytes.argtypes = [i64]
+        L.aw_energy_stats.argtypes = [C.POINTER(AwState), vp, vp]
         L.aw_indicator.argtypes = [C.POINTER(AwState), C.c_int, dbl, vp]
         L.aw_density.argtypes = [C.POINTER(AwState), vp, i32, i32, dbl, dbl, C.c_int, vp]
         L.aw_stage_constants.argtypes = [C.c_int, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
@@ -252,6 +255,21 @@ def aw_indicator(ens, kind, thr=0.0, out=None, stream=None):
                           device=ens.device)
     _check(lib().aw_indicator(C.byref(ens.c), kind, thr, _ptr(out)), "aw_indicator")
     return out[:ens.n]
+
+
+def aw_energy_stats_scratch_bytes(n):
+    return int(lib().aw_energy_stats_scratch_bytes(n))
+
+
+def aw_energy_stats(ens, out=None, stream=None):
+    """8 doubles on the device: live count, max / mean / rms of dH_max, mean / rms of the signed final error,
+    index of the worst trajectory, max |signed error| (include/aw.h)."""
+    ens.bind_stream(stream)
+    scratch = torch.empty((aw_energy_stats_scratch_bytes(ens.n) + 7) // 8, dtype=torch.float64, device=ens.device)
+    if out is None:
+        out = torch.empty((8,), dtype=torch.float64, device=ens.device)
+    _check(lib().aw_energy_stats(C.byref(ens.c), _ptr(scratch), _ptr(out)), "aw_energy_stats")
+    return out
 
 
 def aw_density(ens, hist, lo, hi, mode=0, dropped=None, stream=None):

@@ -354,8 +354,15 @@ int aw_indicator(const aw_state *s, int kind, double thr, void *out_dev) {
   if (!s || !out_dev) return AW_EINVAL;
   int rc = check_planes(s);
   if (rc != AW_OK) return rc;
-  if (kind < AW_IND_FLI || kind > AW_IND_VZ) return AW_EINVAL;
+  if (kind < AW_IND_FLI || kind > AW_IND_DHS) return AW_EINVAL;
   if (!s->ready) return AW_ESTATE;
+  if (kind == AW_IND_DHS) {
+    if (!aligned16(out_dev)) return AW_EINVAL;
+    if (s->n == 0) return AW_OK;
+    AW_CUDA(launch_signed_dh(s->q, s->acc, s->status, s->n, s->pitch, s->eps, static_cast<double *>(out_dev),
+                             (cudaStream_t)s->stream));
+    return AW_OK;
+  }
   if (kind >= AW_IND_DP) {
     if (!has_ref(s)) return AW_ESTATE;
     if (kind != AW_IND_DP && !(s->t > s->tref)) return AW_ESTATE;
@@ -372,6 +379,23 @@ int aw_indicator(const aw_state *s, int kind, double thr, void *out_dev) {
   if (s->n == 0) return AW_OK;
   AW_CUDA(launch_indicator(s->acc, s->status, s->n, s->pitch, kind, thr, s->t, out_dev,
                            (cudaStream_t)s->stream));
+  return AW_OK;
+}
+
+size_t aw_energy_stats_scratch_bytes(int64_t n) {
+  if (n < 0) n = 0;
+  const int64_t nb = energy_stats_blocks(n);
+  return (size_t)(nb > 0 ? nb : 1) * energy_partial_bytes();
+}
+
+int aw_energy_stats(const aw_state *s, void *scratch_dev, double *out_dev) {
+  if (!s || !scratch_dev || !out_dev) return AW_EINVAL;
+  int rc = check_planes(s);
+  if (rc != AW_OK) return rc;
+  if (!aligned16(scratch_dev) || !aligned16(out_dev)) return AW_EINVAL;
+  if (!s->ready) return AW_ESTATE;
+  AW_CUDA(launch_energy_stats(s->q, s->acc, s->status, s->n, s->pitch, s->eps, scratch_dev, out_dev,
+                              (cudaStream_t)s->stream));
   return AW_OK;
 }
 

@@ -85,6 +85,12 @@ cudaError_t launch_hamiltonian_probe(const double *q, int64_t n, int64_t pitch, 
 cudaError_t launch_dfma_peak(int blocks, int threads, int chains, int64_t iters, double *sink,
                              cudaStream_t st);
 
+int64_t energy_stats_blocks(int64_t n);
+size_t energy_partial_bytes();
+cudaError_t launch_energy_stats(const double *q, const double *acc, const uint8_t *status, int64_t n, int64_t pitch,
+                                double eps, void *scratch, double *out, cudaStream_t st);
+cudaError_t launch_signed_dh(const double *q, const double *acc, const uint8_t *status, int64_t n, int64_t pitch,
+                             double eps, double *out, cudaStream_t st);
 cudaError_t launch_dfma_shape(int blocks, int threads, int shape, int64_t iters, double *sink, const double *in,
                               cudaStream_t st);
 

@@ -1,5 +1,6 @@
 // aw_reduce.cu — §8(a) a5 (indicator image) and a6 (visited-cell density histogram); DESIGN.md §6.3-6.4.
 #include "aw_internal.cuh"
+#include "aw_model.cuh"
 
 namespace aw {
 
@@ -78,6 +79,94 @@ __global__ void __launch_bounds__(256) indicator_ref_kernel(const __grid_constan
       if (averaged_velocity(v, k, vh)) r = kind == AW_IND_VX ? vh[0] : (kind == AW_IND_VY ? vh[1] : vh[2]);
     }
   }
+  out[k] = r;
+}
+
+// ------------------------------------------------------------ energy-drift statistics (BJ:configs[2]; R29)
+// Over the live trajectories: count, max / sum / sum of squares of dH_max (acc plane 3), sum / sum of squares /
+// max |.| of the signed error of the current state H(X,P) - H0, and the first index attaining max dH_max.
+// Deterministic: fixed block partials (warp shuffles in a fixed order), then one block folds the partials in a
+// fixed order, so the result does not depend on scheduling (no floating-point atomics).
+struct EnergyPartial {
+  double cnt, mx, idx, sum, sq, ssum, ssq, smax;
+};
+__device__ __forceinline__ void fold(EnergyPartial &a, const EnergyPartial &b) {
+  if (b.cnt > 0.0 && (a.cnt == 0.0 || b.mx > a.mx || (b.mx == a.mx && b.idx < a.idx))) { a.mx = b.mx; a.idx = b.idx; }
+  a.cnt += b.cnt; a.sum += b.sum; a.sq += b.sq; a.ssum += b.ssum; a.ssq += b.ssq;
+  a.smax = fmax(a.smax, b.smax);
+}
+__device__ __forceinline__ EnergyPartial shuffle_down(const EnergyPartial &a, int off) {
+  EnergyPartial b;
+  b.cnt = __shfl_down_sync(0xffffffffu, a.cnt, off); b.mx = __shfl_down_sync(0xffffffffu, a.mx, off);
+  b.idx = __shfl_down_sync(0xffffffffu, a.idx, off); b.sum = __shfl_down_sync(0xffffffffu, a.sum, off);
+  b.sq = __shfl_down_sync(0xffffffffu, a.sq, off); b.ssum = __shfl_down_sync(0xffffffffu, a.ssum, off);
+  b.ssq = __shfl_down_sync(0xffffffffu, a.ssq, off); b.smax = __shfl_down_sync(0xffffffffu, a.smax, off);
+  return b;
+}
+constexpr int kStatsBlock = 256;
+constexpr int kStatsItems = 8;
+
+__device__ __forceinline__ void block_fold(EnergyPartial &a, EnergyPartial *sh) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) { const EnergyPartial b = shuffle_down(a, off); fold(a, b); }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) sh[warp] = a;
+  __syncthreads();
+  if (warp == 0) {
+    EnergyPartial z = {0, 0, -1, 0, 0, 0, 0, 0};
+    a = lane < kStatsBlock / 32 ? sh[lane] : z;
+#pragma unroll
+    for (int off = 4; off > 0; off >>= 1) { const EnergyPartial b = shuffle_down(a, off); fold(a, b); }
+  }
+}
+
+__global__ void __launch_bounds__(kStatsBlock)
+    energy_partial_kernel(const double *__restrict__ q, const double *__restrict__ acc,
+                          const uint8_t *__restrict__ status, int64_t n, int64_t P, double eps,
+                          EnergyPartial *partials) {
+  __shared__ EnergyPartial sh[kStatsBlock / 32];
+  EnergyPartial a = {0, 0, -1, 0, 0, 0, 0, 0};
+  const int64_t base = (int64_t)blockIdx.x * (kStatsBlock * kStatsItems);
+  for (int it = 0; it < kStatsItems; ++it) {
+    const int64_t k = base + (int64_t)it * kStatsBlock + threadIdx.x;
+    if (k < n && status[k] == AW_ST_LIVE) {
+      const double sd = hamiltonian_dev(q[k], q[P + k], q[2 * P + k], q[3 * P + k], q[4 * P + k], q[5 * P + k], eps) -
+                        acc[2 * P + k];
+      const double d = acc[3 * P + k];
+      EnergyPartial b = {1.0, d, (double)k, d, d * d, sd, sd * sd, fabs(sd)};
+      fold(a, b);
+    }
+  }
+  block_fold(a, sh);
+  if (threadIdx.x == 0) partials[blockIdx.x] = a;
+}
+
+__global__ void __launch_bounds__(kStatsBlock)
+    energy_final_kernel(const EnergyPartial *partials, int64_t nblocks, double *out) {
+  __shared__ EnergyPartial sh[kStatsBlock / 32];
+  EnergyPartial a = {0, 0, -1, 0, 0, 0, 0, 0};
+  for (int64_t b = threadIdx.x; b < nblocks; b += kStatsBlock) fold(a, partials[b]);
+  block_fold(a, sh);
+  if (threadIdx.x == 0) {
+    const double nan = __longlong_as_double(0x7ff8000000000000ll);
+    const bool any = a.cnt > 0.0;
+    out[0] = a.cnt; out[1] = a.mx; out[6] = any ? a.idx : -1.0; out[7] = a.smax;
+    out[2] = any ? a.sum / a.cnt : nan;
+    out[3] = any ? sqrt(a.sq / a.cnt) : nan;
+    out[4] = any ? a.ssum / a.cnt : nan;
+    out[5] = any ? sqrt(a.ssq / a.cnt) : nan;
+  }
+}
+
+// signed energy error of the current state, H(X,P) - H0 (NaN where not live)
+__global__ void __launch_bounds__(256) signed_dh_kernel(const double *__restrict__ q, const double *__restrict__ acc,
+                                                        const uint8_t *__restrict__ status, int64_t n, int64_t P,
+                                                        double eps, double *__restrict__ out) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  double r = __longlong_as_double(0x7ff8000000000000ll);
+  if (status[k] == AW_ST_LIVE)
+    r = hamiltonian_dev(q[k], q[P + k], q[2 * P + k], q[3 * P + k], q[4 * P + k], q[5 * P + k], eps) - acc[2 * P + k];
   out[k] = r;
 }
 
@@ -240,6 +329,32 @@ cudaError_t launch_dfma_shape(int blocks, int threads, int shape, int64_t iters,
 cudaError_t launch_indicator(const double *acc, const uint8_t *status, int64_t n, int64_t pitch, int kind,
                              double thr, double t, void *out, cudaStream_t st) {
   indicator_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(acc, status, n, pitch, kind, thr, t, out);
+  count_launch();
+  return cudaGetLastError();
+}
+
+int64_t energy_stats_blocks(int64_t n) {
+  const int64_t per = (int64_t)kStatsBlock * kStatsItems;
+  return (n + per - 1) / per;
+}
+size_t energy_partial_bytes() { return sizeof(EnergyPartial); }
+
+cudaError_t launch_energy_stats(const double *q, const double *acc, const uint8_t *status, int64_t n, int64_t pitch,
+                                double eps, void *scratch, double *out, cudaStream_t st) {
+  const int64_t nb = energy_stats_blocks(n);
+  EnergyPartial *part = static_cast<EnergyPartial *>(scratch);
+  if (nb > 0) {
+    energy_partial_kernel<<<(unsigned)nb, kStatsBlock, 0, st>>>(q, acc, status, n, pitch, eps, part);
+    count_launch();
+  }
+  energy_final_kernel<<<1, kStatsBlock, 0, st>>>(part, nb, out);
+  count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_signed_dh(const double *q, const double *acc, const uint8_t *status, int64_t n, int64_t pitch,
+                             double eps, double *out, cudaStream_t st) {
+  signed_dh_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(q, acc, status, n, pitch, eps, out);
   count_launch();
   return cudaGetLastError();
 }

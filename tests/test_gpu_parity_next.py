@@ -418,3 +418,38 @@ def test_full_horizon_indicator_map_parity(aw, orc, cfgk, nsample):
     # energy: bounded, no secular growth on every live pixel of the full image
     dH = aw.aw_indicator(ens, aw.AW_IND_DH).cpu().numpy()
     assert np.nanmax(dH) < 1e-8
+
+
+# ------------------------------------------------------------------ energy-drift statistics (configs[2])
+
+@pytest.mark.parametrize("gx,gy", [(1, 1), (67, 33), (512, 301)])
+def test_energy_drift_statistics_parity(aw, orc, gx, gy):
+    """BASELINE configs[2] outputs "indicator image and energy-drift statistics": aw_energy_stats and the signed
+    dH image against the oracle on the same device state.  Integer-like entries (count, worst index) and the
+    maxima of stored values are exact; sums differ by the summation order (1e-12 relative); the signed error is
+    H - H0 by each side's own H routine (device sincos vs libm: a few ulp(E))."""
+    cfg = aw.CONFIGS[2]
+    n = gx * gy
+    ens = aw.Ensemble(n, tangent=True, wind=True)
+    aw.aw_init_shell(ens, aw.make_grid(gx, gy, -1.02, 1.02, angle_mode=1), cfg["E"], 1e-2, cfg["seed"])
+    aw.aw_integrate(ens, n, 500, cfg["dt"], cfg["stride"])
+    out = aw.aw_energy_stats(ens).cpu().numpy()
+    out2 = aw.aw_energy_stats(ens).cpu().numpy()
+    assert np.array_equal(out, out2, equal_nan=True)                     # deterministic reduction
+    img = aw.aw_indicator(ens, aw.AW_IND_DHS).cpu().numpy()
+    st = ensemble_to_oracle(ens, orc)
+    ref, ref_img = orc.energy_stats(st)
+    live = st.status == 1
+    ulpE = 2.0 ** -52 * cfg["E"]
+    assert np.array_equal(np.isnan(img), ~live)
+    assert np.max(np.abs(img[live] - ref_img[live]), initial=0.0) <= 8 * ulpE
+    assert out[0] == ref[0] == live.sum()
+    if live.sum() == 0:
+        assert np.isnan(out[2]) and out[6] == -1
+        return
+    assert out[1] == ref[1] and out[6] == ref[6]
+    assert abs(out[2] - ref[2]) <= 1e-12 * ref[2] and abs(out[3] - ref[3]) <= 1e-12 * ref[3]
+    assert abs(out[4] - ref[4]) <= 8 * ulpE and abs(out[5] - ref[5]) <= 8 * ulpE
+    assert abs(out[7] - ref[7]) <= 8 * ulpE
+    # the numbers themselves: 4th order at dt = 0.02 keeps |dH| ~ 1e-9, no drift of the mean (P:55)
+    assert out[1] < 1e-7 and abs(out[4]) <= out[5]
