@@ -315,6 +315,7 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
   double amax = std::fabs(p.a_open);
   for (int k = 0; k < S; ++k) amax = std::fmax(amax, std::fabs(p.a_loop[k]));
   p.level = s->trig ? 0 : trig_level_for(amax * vmax);
+  if (p.level > 0 && (amax != std::fabs(p.a_loop[S - 1]) || !drift_ratios_hold(S, p.a_loop))) p.level = 0;
   const int64_t pieces = (stride + kMaxChunk - 1) / kMaxChunk;
   p.chunk = (int32_t)((stride + pieces - 1) / pieces);
 

@@ -101,17 +101,31 @@ __device__ __forceinline__ void rotate(double &s, double &c, double g, double m)
   c = c1;
 }
 
-// Degrees (u/v pairs, 2z pair) of the trigonometry levels.  With |d| = max_s |a_s| max|P| the u and v pairs see
-// angles up to sqrt(2) |d| (|px +- py| <= sqrt(2) |P|), the 2z pair up to 2 |d| (trig_level_for).
-template <int LEVEL> struct Deg;
-template <> struct Deg<0> { static constexpr int uv = 1, z = 1; };  // unused
-template <> struct Deg<1> { static constexpr int uv = 3, z = 3; };
-template <> struct Deg<2> { static constexpr int uv = 3, z = 4; };
-template <> struct Deg<3> { static constexpr int uv = 4, z = 4; };
-template <> struct Deg<4> { static constexpr int uv = 4, z = 5; };
-template <> struct Deg<5> { static constexpr int uv = 5, z = 6; };
-template <> struct Deg<6> { static constexpr int uv = 6, z = 7; };
-template <> struct Deg<7> { static constexpr int uv = 7, z = 8; };
+// Taylor degrees of the drift rotations.  A trigonometry level L is picked on the host from
+// |d| = max_s |a_s| max|P| <= kLevelMaxD[L] (trig_level_for).  The drift after kick s has its own constant
+// a_loop[s]; its ratio to the largest one is fixed by the scheme (kDriftRatio, checked on the host), so each
+// drift gets the smallest degree N whose truncation stays below 2^-60 for ITS largest angle: the u and v pairs
+// rotate by up to sqrt(2) |a_loop[s]| max|P|, the zeta = 2z pair by up to 2 |a_loop[s]| max|P|, and a degree-N
+// pair truncates at t^(2N+2)/(2N+2)! (cos - 1; the sine's t^(2N+3)/(2N+3)! is smaller) for an angle t:
+//   N = 1: t <= 6.8e-5;  2: 0.00293;  3: 0.0208;  4: 0.0708;  5: 0.165;  6: 0.310;  7: 0.505;  8: 0.750.
+// The largest drift (the merged one) gets degrees (3,3), (3,4), (4,4), (4,5), (5,6), (6,7), (7,8) at levels
+// 1..7; the short inner drifts of the triple jump (ratio 0.13) and of the 7-stage scheme (0.088) one or two less.
+constexpr double kLevelMaxD[8] = {0.0, 0.0104, 0.0147, 0.0354, 0.0500, 0.1166, 0.2192, 0.3570};
+constexpr double kDegreeMaxAngle[9] = {0.0, 6.8e-5, 0.00293, 0.0208, 0.0708, 0.165, 0.310, 0.505, 0.750};
+
+// upper bounds of |a_loop[cs]| / max_s |a_loop[s]| for the coefficient sets cs of drift() (cs = S-1: merged drift)
+template <int S> struct DriftRatio;
+template <> struct DriftRatio<3> { static constexpr double r[3] = {0.1300, 0.1300, 1.0}; };
+template <> struct DriftRatio<7> { static constexpr double r[7] = {0.6502, 0.6005, 0.08765, 0.08765, 0.6005, 0.6502, 1.0}; };
+
+template <int S, int LEVEL, int cs, bool ZETA>
+__host__ __device__ constexpr int rotation_degree() {
+  if (LEVEL == 0) return 1;  // unused
+  const double t = (ZETA ? 2.0 : 1.4142135623730951) * kLevelMaxD[LEVEL] * DriftRatio<S>::r[cs];
+  int n = 1;
+  while (n < 8 && kDegreeMaxAngle[n] < t) ++n;
+  return n;
+}
 
 // Everything a thread carries between stages.  Inside a block of `stride` steps the state is held in the
 // rotated and scaled variables
@@ -179,20 +193,21 @@ template <int S, bool TAN, int LEVEL, int s>
 __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
   constexpr int cs = (s == S - 1) ? s : (s < S - 2 - s ? s : S - 2 - s);
   if (LEVEL > 0) {
+    constexpr int nuv = rotation_degree<S, LEVEL, cs, false>(), nz = rotation_degree<S, LEVEL, cs, true>();
     double g, m;
     if (S <= 3) {
-      small_sincos<Deg<LEVEL>::uv>(t.pu, p.grot[cs], p.mrot[cs], g, m);
+      small_sincos<nuv>(t.pu, p.grot[cs], p.mrot[cs], g, m);
       rotate(t.su, t.cu, g, m);
-      small_sincos<Deg<LEVEL>::uv>(t.pv, p.grot[cs], p.mrot[cs], g, m);
+      small_sincos<nuv>(t.pv, p.grot[cs], p.mrot[cs], g, m);
       rotate(t.sv, t.cv, g, m);
-      small_sincos<Deg<LEVEL>::z>(t.pzt, p.grot[cs], p.mrot[cs], g, m);
+      small_sincos<nz>(t.pzt, p.grot[cs], p.mrot[cs], g, m);
       rotate(t.s2, t.c2, g, m);
     } else {
-      small_sincos_angle<Deg<LEVEL>::uv>(p.a_loop[cs] * t.pu, g, m);
+      small_sincos_angle<nuv>(p.a_loop[cs] * t.pu, g, m);
       rotate(t.su, t.cu, g, m);
-      small_sincos_angle<Deg<LEVEL>::uv>(p.a_loop[cs] * t.pv, g, m);
+      small_sincos_angle<nuv>(p.a_loop[cs] * t.pv, g, m);
       rotate(t.sv, t.cv, g, m);
-      small_sincos_angle<Deg<LEVEL>::z>(p.a_loop[cs] * t.pzt, g, m);
+      small_sincos_angle<nz>(p.a_loop[cs] * t.pzt, g, m);
       rotate(t.s2, t.c2, g, m);
     }
   }
@@ -361,14 +376,20 @@ cudaError_t launch_level(const IntegrateParams &p, cudaStream_t st) {
 //   also cheaper from there on: a degree-(8,9) rotation costs more fp64 instructions than the sincos it replaces.
 int trig_level_for(double d) {
   if (!(d == d)) return 0;
-  if (d <= 0.0104) return 1;
-  if (d <= 0.0147) return 2;
-  if (d <= 0.0354) return 3;
-  if (d <= 0.0500) return 4;
-  if (d <= 0.1166) return 5;
-  if (d <= 0.2192) return 6;
-  if (d <= 0.3570) return 7;
+  for (int level = 1; level <= 7; ++level)
+    if (d <= kLevelMaxD[level]) return level;
   return 0;
+}
+
+// The per-drift degrees assume the ratios |a_loop[cs]| / max |a_loop| of the two built-in stage lists.
+bool drift_ratios_hold(int S, const double *a_loop) {
+  double amax = 0.0;
+  for (int s = 0; s < S; ++s) amax = fmax(amax, fabs(a_loop[s]));
+  for (int s = 0; s < S; ++s) {
+    const double r = (S == 3) ? DriftRatio<3>::r[s] : DriftRatio<7>::r[s];
+    if (fabs(a_loop[s]) > r * amax) return false;
+  }
+  return true;
 }
 
 cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, cudaStream_t st) {

@@ -58,6 +58,8 @@ struct InitParams {
 cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, cudaStream_t st);
 // Trigonometry variant for a largest drift angle max_s |a_s| * max|p| (0 = full sincos every stage).
 int trig_level_for(double max_drift_angle);
+// true if |a_loop[s]| / max |a_loop| are within the ratios the per-drift Taylor degrees were derived for
+bool drift_ratios_hold(int S, const double *a_loop);
 constexpr int kMaxChunk = 128;
 cudaError_t launch_init(const InitParams &p, cudaStream_t st);
 cudaError_t launch_indicator(const double *acc, const uint8_t *status, int64_t n, int64_t pitch, int kind,
