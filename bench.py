@@ -48,6 +48,8 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--density-bench", action="store_true",
+                    help="only time aw_density / aw_init_shell / aw_indicator alone (HBM-bound kernels, DESIGN.md 6.3-6.4)")
     ap.add_argument("--dfma-shapes", action="store_true",
                     help="only run the fp64 operand-shape probe (aw_dfma_shape_probe) and print its JSON line")
     return ap.parse_args()
@@ -400,10 +402,65 @@ def run_dfma_shapes():
     print(json.dumps({"probe": "aw_dfma_shape_probe", "sms": sms, "shapes": out}), flush=True)
 
 
+def run_density_bench():
+    """The HBM-bound kernels alone (SURVEY 8(d): the histogram on clustered and on spread input, 2^20 and 2^22 points;
+    init_shell; indicator), CUDA events over 20 back-to-back launches each, against the measured HBM copy bandwidth."""
+    import torch
+    from paper_1107_4107_b200 import build as awbuild
+    awbuild.build()
+    import paper_1107_4107_b200 as aw
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm = peaks.get("hbm_gbs")
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, reps=20):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3 / reps
+
+    rows = []
+    for logn in (20, 22):
+        g = 1 << (logn // 2)
+        n = g * g
+        ens = aw.Ensemble(n, tangent=True, wind=True, ref=True)
+        hist = torch.zeros((1024, 1024), dtype=torch.int32, device="cuda")
+        dropped = torch.zeros(1, dtype=torch.int64, device="cuda")
+        image = torch.empty(n, dtype=torch.float64, device="cuda")
+        for label, grid, eps in (("clustered: disk r = 1e-3 at (0,0), <= 4 bins", aw.make_grid(g, g, -1.0, 1.0, 1, 1, 0.0, 0.0, 1e-3), 1e-3),
+                                 ("spread: cell-centred grid over [-1,1]^2", aw.make_grid(g, g, -1.0, 1.0, 0, 0), 3e-2)):
+            t_init = timed(lambda: aw.aw_init_shell(ens, grid, 1.0, eps, 0))
+            aw.aw_mark(ens)
+            aw.aw_integrate(ens, n, 100, 0.005, 100)
+            t_act = timed(lambda: aw.aw_density(ens, hist, -1.0, 1.0, 0, dropped))
+            t_vel = timed(lambda: aw.aw_density(ens, hist, -1.5, 1.5, 3, dropped))
+            t_ind = timed(lambda: aw.aw_indicator(ens, aw.AW_IND_FLI, 0.0, out=image))
+            b_init = n * (48 + 48 + 32 + 12 + 1)            # bytes written per trajectory (DESIGN.md 6.3)
+            rows.append({"n": n, "input": label,
+                         "init_shell_us": t_init * 1e6, "init_shell_GBs": b_init / t_init / 1e9,
+                         "density_action_us": t_act * 1e6, "density_action_GBs": n * 17 / t_act / 1e9,
+                         "density_velocity_us": t_vel * 1e6, "density_velocity_GBs": n * 73 / t_vel / 1e9,
+                         "indicator_us": t_ind * 1e6, "indicator_GBs": n * 17 / t_ind / 1e9})
+    print(json.dumps({"probe": "hbm_bound_kernels", "hbm_copy_peak_GBs": hbm,
+                      "bytes_per_trajectory": {"init_shell": 141, "density_action": 17, "density_velocity": 73,
+                                               "indicator": 17}, "rows": rows}), flush=True)
+
+
 def main():
     args = parse()
     if args.dfma_shapes:
         return run_dfma_shapes()
+    if args.density_bench:
+        return run_density_bench()
     from paper_1107_4107_b200.configs import CONFIGS
     cfg = dict(CONFIGS[args.config])
     order = args.order or cfg["order"]
