@@ -3,31 +3,37 @@
 // One trajectory per thread ("complete parallelisation"); the six state words, the six tangent
 // words and the running (sin, cos) pairs live in registers for the whole launch; HBM is touched at launch
 // start and end, plus one read-modify-write of the accumulator planes per checkpoint.  The stage loop is
-// fully unrolled so a_s, b_s, 2b_s, 4b_s are constant-bank operands.  Bound by the fp64 pipe.
+// fully unrolled; the stage constants reach the fp64 instructions through uniform registers.  Bound by the
+// fp64 pipe.
 //
 // Scheme (ref. 25; R2): for s = 1..S { X += a_s P ; P -= b_s grad H_p(X) }  X += a_{S+1} P.
 // Inside a block of `stride` steps the closing drift of a step and the opening drift of the next are
 // one FMA with the constant a_{S+1} + a_1 (same map, one rounding fewer; DESIGN.md §7 D3).  A block is
 //   X += a_1 P;  stride x { for s: kick_s; X += a_loop[s] P };  X -= a_1 P;  checkpoint
 // (a_1 = a_{S+1} for the palindromic stage lists, so the last merged drift minus a_1 P is the closing drift).
-// Model (eq. 2) with F = 1 + cos 2z:  H_p = cx cy F,
-//   grad H_p = (-sx cy F, -cx sy F, -2 cx cy sin 2z),  Hessian in SURVEY.md Appendix A.2.
 //
-// Trigonometry.  LEVEL 0: the device sincos (aw_trig.cuh) of x, y, z at every stage.
-// LEVEL >= 1: the pairs (sin x, cos x), (sin y, cos y), (sin 2z, cos 2z) are carried in registers and
-// advanced through every drift X += a P by the rotation with the drift angle d = a p (2 a pz for 2z):
+// Model (eq. 2): H_p = cos x cos y (1 + cos 2z) = (cos u + cos v)(1 + cos zeta)/2 in the working
+// variables u = x + y, v = x - y, zeta = 2z the kernel holds inside a block (struct Traj below), so
+//   grad H_p = -(F sin u, F sin v, (cos u + cos v) sin zeta),  F = 1 + cos zeta   (d/du, d/dv, d/dz),
+// and the Hessian-vector product is the sum and difference of the x and y rows of SURVEY.md Appendix A.2.
+//
+// Trigonometry.  LEVEL 0: the device sincos (aw_trig.cuh) of u, v, zeta at every stage.
+// LEVEL >= 1: the pairs (sin u, cos u), (sin v, cos v), (sin zeta, cos zeta) are carried in registers and
+// advanced through every drift by the rotation with the drift angle d = a p (p = pu, pv, pzeta):
 //     s' = s + (s m + c g),  c' = c + (c m - s g),   g = sin d = p G(p^2),  m = cos d - 1 = p^2 M(p^2),
 // G and M being the Taylor polynomials of sin and cos - 1 with the powers of a folded into their
-// coefficients on the host (constant-bank operands); the degree is picked on the host from the largest
-// possible |d| so that the truncation error stays below 2^-60 (trig_level_for).  The pairs are
-// re-synchronised from the tracked angles with the full sincos after the opening drift of every block and
-// at least every kMaxChunk steps, which bounds the rounding random walk of the rotations at a few 1e-15.
+// coefficients on the host; the degree of every drift is fixed at compile time from the level the host picks
+// (largest possible |d|) and the drift's ratio to the largest one, so that the truncation error stays below
+// 2^-60 (rotation_degree, trig_level_for).  The pairs are re-synchronised from the tracked angles with the
+// full sincos after the opening drift of every block and at least every kMaxChunk steps, which bounds the
+// rounding random walk of the rotations at a few 1e-15.
 //
 // Instruction shapes (profiles/r1c_dfma_operand_shapes.md): on sm_100 a DFMA that reads three distinct 64-bit
-// registers issues every 3 cycles instead of 2 unless one operand comes from the operand-reuse cache, the
-// constant bank or an immediate.  The code below therefore keeps polynomial coefficients and stage
-// constants in the constant bank and writes the remaining three-register FMAs in groups that share an
-// operand in the same slot (the rotation's g, the kick's F, the tangent map's column vector).
+// registers issues every 3 cycles instead of 2 unless one operand comes from the operand-reuse cache, a
+// uniform register or an immediate, and every non-fp64 instruction takes an issue cycle the fp64 pipe also
+// needs.  The code below therefore minimises register reads and integer work, not just fp64 instructions:
+// coefficients and stage constants in uniform registers, the working variables above (16 three-register
+// multiply-adds per stage instead of 21), three-register FMAs written in groups that share an operand.
 #include <cmath>
 
 #include "aw_internal.cuh"
@@ -55,7 +61,7 @@ __device__ __forceinline__ double wrap_angle(double x, int &turns) {
   return fma(-k, kTwoPiLo, fma(-k, kTwoPiHi, x));
 }
 
-// g = sin(A p), m = cos(A p) - 1 as p G(z), z M(z), z = p^2: N + (N-1) FMA with constant-bank coefficients,
+// g = sin(A p), m = cos(A p) - 1 as p G(z), z M(z), z = p^2: N + (N-1) FMA with uniform-register coefficients,
 // 3 DMUL.  Truncation: |d|^(2N+3)/(2N+3)! in g, |d|^(2N+2)/(2N+2)! in m (d = A p).
 template <int N>
 __device__ __forceinline__ void small_sincos(double p, const double (&G)[kTrigTerms + 1],
