@@ -453,3 +453,51 @@ def test_energy_drift_statistics_parity(aw, orc, gx, gy):
     assert abs(out[7] - ref[7]) <= 8 * ulpE
     # the numbers themselves: 4th order at dt = 0.02 keeps |dH| ~ 1e-9, no drift of the mean
     assert out[1] < 1e-7 and abs(out[4]) <= out[5]
+
+
+# ------------------------------------------------------------------ large ragged ensemble
+
+def test_large_ragged_ensemble_sampled_parity(aw, orc):
+    """2^25 + 17 trajectories (8 x the 2048 x 2048 scan, 262 145 blocks, ragged tail): init, 200 steps with the
+    tangent map, FLI image and histogram; parity on 600 sampled trajectories (first, last, block edges, hashed),
+    gathered on the device so that only the sample crosses to the host."""
+    gx, gy = (1 << 25) + 17, 1
+    n = gx * gy
+    ens = aw.Ensemble(n, tangent=True, wind=True, order=4)
+    assert ens.pitch == n + 15 and ens.pitch % 32 == 0
+    aw.aw_init_shell(ens, aw.make_grid(gx, gy, -0.9, 0.9, angle_mode=1, lo_y=0.3, hi_y=0.5), 1.0, 3e-2, 99)
+    hashed = [orc.mix64(25, i) % n for i in range(560)]
+    sample = np.unique(np.array([0, 1, 127, 128, 129, n - 1, n - 2, n - 17, n - 18, n // 2] + hashed, dtype=np.int64))
+    idx = torch.from_numpy(sample).cuda()
+    m = len(sample)
+
+    def grab():
+        st = orc.State(m, tangent=True, wind=True)
+        st.q[:, :m] = ens.q[:, idx].cpu().numpy()
+        st.w[:, :m] = ens.w[:, idx].cpu().numpy()
+        st.acc[:, :m] = ens.acc[:, idx].cpu().numpy()
+        st.wind[:, :m] = ens.wind[:, idx].cpu().numpy()
+        st.status[:] = ens.status[idx].cpu().numpy()
+        st.E, st.eps, st.t, st.step, st.order = ens.E, ens.eps, ens.t, ens.step, ens.order
+        return st
+
+    st = grab()
+    assert np.all(st.status == 1)
+    aw.aw_integrate(ens, n, 200, 0.005, 100)
+    orc.integrate(st, 200, 0.005, 100)
+    got = grab()
+    err = state_rel_err(got.q[:, :m], got.wind[:, :m], st.q[:, :m], st.wind[:, :m], np.ones(m, bool))
+    assert err.max() <= 1e-10, err.max()
+    assert np.max(np.abs(got.acc[1, :m] - st.acc[1, :m])) <= 1e-5
+    fli = aw.aw_indicator(ens, aw.AW_IND_FLI)
+    assert torch.equal(fli[idx].cpu(), torch.from_numpy(got.acc[1, :m].copy()))
+    assert bool(torch.isfinite(fli).all())
+    hist = torch.zeros((64, 64), dtype=torch.int32, device="cuda")
+    dropped = torch.zeros(1, dtype=torch.int64, device="cuda")
+    aw.aw_density(ens, hist, -1.0, 1.0, 0, dropped)
+    assert int(hist.sum().item()) + int(dropped.item()) == n and int(dropped.item()) == 0
+    # all points sit in the strip 0.3 <= py < 0.5 (+- the kick amplitude): rows 41..47 of the 64-row histogram
+    rows = hist.sum(dim=1).cpu().numpy()
+    assert rows[:40].sum() == 0 and rows[49:].sum() == 0
+    stats = aw.aw_energy_stats(ens).cpu().numpy()
+    assert stats[0] == n and stats[1] < 1e-9
