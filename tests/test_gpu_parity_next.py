@@ -501,3 +501,47 @@ def test_large_ragged_ensemble_sampled_parity(aw, orc):
     assert rows[:40].sum() == 0 and rows[49:].sum() == 0
     stats = aw.aw_energy_stats(ens).cpu().numpy()
     assert stats[0] == n and stats[1] < 1e-9
+
+
+# ------------------------------------------------------------------ closed forms on the GPU (pins P15, P17)
+
+@pytest.mark.parametrize("order", [4, 6])
+def test_gpu_velocity_closed_forms(aw, order):
+    """eps = 0: the averaged velocity over any window is the momentum, its projection too (P^2 = 2E), dP = 0,
+    and the sphere density equals the action density of the same state bin for bin.  Pendulum subspace
+    (y = z = py = pz = 0): over 5 rotation periods V_x = 2 pi / T(h), T from the complete elliptic integral."""
+    from scipy.special import ellipk
+    n = 60 * 50        # cell centres = centres of the 64-bin histogram below (bin width 1/32): no edge cases
+    ens = aw.Ensemble(n, tangent=False, wind=True, order=order, ref=True)
+    aw.aw_init_shell(ens, aw.make_grid(60, 50, -60 / 64, 60 / 64, angle_mode=1, lo_y=-50 / 64, hi_y=50 / 64),
+                     1.0, 0.0, 3)
+    aw.aw_integrate(ens, n, 300, 0.01, 100)
+    aw.aw_mark(ens)
+    aw.aw_integrate(ens, n, 20000, 0.01, 100)                 # Dt = 200: ~45 whole turns
+    P = ens.q[3:6, :n].cpu().numpy()
+    V = np.stack([aw.aw_indicator(ens, k).cpu().numpy() for k in (aw.AW_IND_VX, aw.AW_IND_VY, aw.AW_IND_VZ)])
+    assert int(ens.wind.abs().max().item()) > 20
+    assert np.max(np.abs(V - P)) < 1e-12
+    assert float(aw.aw_indicator(ens, aw.AW_IND_DP).max().item()) == 0.0
+    ha = torch.zeros((64, 64), dtype=torch.int32, device="cuda")
+    hv = torch.zeros((64, 64), dtype=torch.int32, device="cuda")
+    aw.aw_density(ens, ha, -1.0, 1.0, aw.AW_DENS_ACTION)
+    aw.aw_density(ens, hv, -1.0, 1.0, aw.AW_DENS_VEL_UPPER)
+    assert torch.equal(ha, hv) and int(ha.sum().item()) == n
+    # pendulum
+    eps, px0 = 1e-2, 1.0
+    h = 0.5 * px0 ** 2 + 2 * eps
+    T = 4 * ellipk(4 * eps / (h + 2 * eps)) / math.sqrt(2 * (h + 2 * eps))
+    pen = aw.Ensemble(32, tangent=False, wind=True, order=order, ref=True)
+    q = np.zeros((6, pen.pitch)); q[3, :32] = px0
+    acc = np.zeros((4, pen.pitch)); acc[2, :32] = h
+    pen.load_host(q, None, acc, np.zeros((3, pen.pitch), dtype=np.int32), np.ones(32, dtype=np.uint8), h, eps)
+    aw.aw_mark(pen)
+    aw.aw_integrate(pen, 32, 5000, 5 * T / 5000, 100)
+    vx = aw.aw_indicator(pen, aw.AW_IND_VX).cpu().numpy()
+    assert np.max(np.abs(vx - math.sqrt(2 * h))) < 1e-12       # projected: V is along x, |Vhat| = sqrt(2E), E = h
+    qf = pen.q.cpu().numpy()
+    X = qf[0, :32] + 2 * math.pi * pen.wind[0, :32].cpu().numpy()
+    tol = 1e-8 if order == 4 else 1e-10
+    assert np.max(np.abs(X / (5 * T) - 2 * math.pi / T)) < tol
+    assert np.all(qf[[1, 2, 4, 5], :32] == 0.0)               # the invariant subspace, exactly
