@@ -299,6 +299,10 @@ def run_ours(args, cfg, order, tangent):
                 "frac": achieved / FP64_PEAK_TFLOPS_NOMINAL, "traffic": traffic, "traffic_source": traffic_src,
                 "peak_source": "derived: 148 SM x 64 DFMA/clk/SM x 2 flop x 1.965 GHz (DESIGN.md §6.1); "
                                "MEASURED_PEAKS.json has no fp64 entry",
+                # SURVEY 8(d) reporting rule: the smaller of the nominal accounting figure and the executed flops;
+                # at the nominal figure the same run would read achieved_at_nominal_flops (can exceed the peak:
+                # the kernel does the step's work in fewer flops than the accounting convention assumes)
+                "achieved_at_nominal_flops": kernel_rate * flops_nominal / 1e12,
                 "flops_per_traj_step": flops_per_step, "flops_per_traj_step_nominal": flops_nominal,
                 "flops_per_traj_step_executed": mix["flops"],
                 "sass_per_step": {k: mix[k] for k in ("dfma", "dmul", "dadd", "other")},
