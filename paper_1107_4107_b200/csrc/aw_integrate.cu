@@ -43,8 +43,12 @@
 #ifndef AW_BLOCK
 #define AW_BLOCK 128
 #endif
+// Register cap: __launch_bounds__(128, 3) allows 168 registers per thread; the kernels take 102-134, which still
+// places 4 (order 6 without tangent at the high levels: 3) blocks per SM, and 3 warps per sub-partition already
+// saturate the fp64 pipe.  With the cap at 128 ptxas finds fewer operand-reuse pairs in most instantiations
+// (measured: configs[3] -1.1 %), except the level-4 ones (configs[2]: +1.8 % at 128), which keep 4.
 #ifndef AW_MIN_BLOCKS
-#define AW_MIN_BLOCKS 4
+#define AW_MIN_BLOCKS(LEVEL) ((LEVEL) == 4 ? 4 : 3)
 #endif
 
 namespace aw {
@@ -270,7 +274,7 @@ __device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p) {
 }
 
 template <int S, bool TAN, int LEVEL>
-__global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS)
+__global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS(LEVEL))
     integrate_kernel(const __grid_constant__ IntegrateParams p) {
   const int64_t k = (int64_t)blockIdx.x * AW_BLOCK + threadIdx.x;
   if (k >= p.n) return;
