@@ -12,6 +12,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libaw.so")
 SOURCES = ["aw_api.cu", "aw_integrate.cu", "aw_init.cu", "aw_reduce.cu"]
+# (source, object, extra flags): aw_integrate.cu is compiled a second time for the kernels of trig levels 1-4 with
+# ptxas -O1, whose scheduling keeps operand-sharing FMAs adjacent (see the comment at AW_LEVEL_GROUP in the source)
+UNITS = [("aw_api.cu", "aw_api.o", []), ("aw_integrate.cu", "aw_integrate.o", []),
+         ("aw_integrate.cu", "aw_integrate_low.o", ["-DAW_LEVEL_GROUP=1", "-Xptxas", "-O1"]),
+         ("aw_init.cu", "aw_init.o", []), ("aw_reduce.cu", "aw_reduce.o", [])]
 HEADERS = ["aw_internal.cuh", "aw_trig.cuh", "aw_trig_coeffs.h", "aw_model.cuh", os.path.join("..", "..", "include", "aw.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-Xptxas", "-v"]
@@ -40,9 +45,9 @@ def build(force=False, verbose=False, extra_flags=()):
     build_dir = os.path.join(HERE, "build")
     os.makedirs(build_dir, exist_ok=True)
     log = []
-    for src in SOURCES:
-        obj = os.path.join(build_dir, src.replace(".cu", ".o"))
-        cmd = [_nvcc()] + NVCC_FLAGS + list(extra_flags) + ["-c", os.path.join(CSRC, src), "-o", obj]
+    for src, objname, unit_flags in UNITS:
+        obj = os.path.join(build_dir, objname)
+        cmd = [_nvcc()] + NVCC_FLAGS + unit_flags + list(extra_flags) + ["-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         log.append(r.stderr)
         if r.returncode != 0:

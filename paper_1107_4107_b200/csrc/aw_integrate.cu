@@ -51,6 +51,15 @@
 #define AW_MIN_BLOCKS(LEVEL) ((LEVEL) == 4 ? 4 : 3)
 #endif
 
+// This file is compiled twice (build.py).  AW_LEVEL_GROUP 1 instantiates the kernels of trig levels 1-4 and is
+// compiled with -Xptxas -O1: ptxas's lighter scheduler keeps the three-register FMAs that share an operand next
+// to each other, so more of them hit the operand-reuse cache (measured on B200: configs[3] +3.5 %, configs[2]
+// +3.5 %, order 6 +2.9 %, configs[4] +1.5 %).  AW_LEVEL_GROUP 0 (default flags) holds levels 0 and 5-7, which
+// lose 2-3 % at -O1, and the host-side functions.
+#ifndef AW_LEVEL_GROUP
+#define AW_LEVEL_GROUP 0
+#endif
+
 namespace aw {
 
 namespace {
@@ -362,18 +371,31 @@ cudaError_t launch_one(const IntegrateParams &p, cudaStream_t st) {
 template <int S, bool TAN>
 cudaError_t launch_level(const IntegrateParams &p, cudaStream_t st) {
   switch (p.level) {
+#if AW_LEVEL_GROUP == 1
     case 1: return launch_one<S, TAN, 1>(p, st);
     case 2: return launch_one<S, TAN, 2>(p, st);
     case 3: return launch_one<S, TAN, 3>(p, st);
     case 4: return launch_one<S, TAN, 4>(p, st);
+    default: return cudaErrorInvalidValue;
+#else
     case 5: return launch_one<S, TAN, 5>(p, st);
     case 6: return launch_one<S, TAN, 6>(p, st);
     case 7: return launch_one<S, TAN, 7>(p, st);
     default: return launch_one<S, TAN, 0>(p, st);
+#endif
   }
 }
 
 }  // namespace
+
+#if AW_LEVEL_GROUP == 1
+
+cudaError_t launch_integrate_low(const IntegrateParams &p, int order, bool tangent, cudaStream_t st) {
+  if (order == 4) return tangent ? launch_level<3, true>(p, st) : launch_level<3, false>(p, st);
+  return tangent ? launch_level<7, true>(p, st) : launch_level<7, false>(p, st);
+}
+
+#else
 
 // Largest |d| = max_s |a_s| max|P| each level may see, with both Taylor truncations below 2^-60 ~ 8.7e-19 (they
 // are systematic, so 300 of them still sum to < 3e-16):
@@ -402,7 +424,10 @@ bool drift_ratios_hold(int S, const double *a_loop) {
   return true;
 }
 
+cudaError_t launch_integrate_low(const IntegrateParams &p, int order, bool tangent, cudaStream_t st);
+
 cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, cudaStream_t st) {
+  if (p.level >= 1 && p.level <= 4) return launch_integrate_low(p, order, tangent, st);
   if (order == 4) return tangent ? launch_level<3, true>(p, st) : launch_level<3, false>(p, st);
   return tangent ? launch_level<7, true>(p, st) : launch_level<7, false>(p, st);
 }
@@ -418,5 +443,7 @@ cudaError_t launch_hamiltonian_probe(const double *q, int64_t n, int64_t pitch, 
   count_launch();
   return cudaGetLastError();
 }
+
+#endif  // AW_LEVEL_GROUP
 
 }  // namespace aw
