@@ -244,6 +244,15 @@ AW_API int aw_map_host(aw_state *s, const aw_host_in *in, int64_t steps, double 
                 double thr, int32_t gx, int32_t gy, double lo, double hi, void *ind_dev,
                 void *hist_dev, const aw_host_out *out);
 
+/* The paper's own pipeline end to end with HOST buffers (synchronous): uploads the host-resident state as
+ * aw_map_host does, takes the snapshot (aw_mark: the state is the X(t) of the window), runs aw_integrate(steps, dt,
+ * stride) — the averaging window Dt = steps*|dt| — then aw_density(mode 1..3) of the projected averaged velocity into
+ * the zeroed device histogram, and downloads it (gx*gy uint32) plus out->dropped / q / acc / status where non-NULL;
+ * out->image is ignored.  hist_dev: device scratch of gx*gy*4 + 8 bytes.  s must carry qref (and windref iff wind). */
+AW_API int aw_velocity_map_host(aw_state *s, const aw_host_in *in, int64_t steps, double dt, int64_t stride, int mode,
+                                int32_t gx, int32_t gy, double lo, double hi, void *hist_dev,
+                                const aw_host_out *out);
+
 /* Probes (synchronous; test and measurement support, not on the hot path) ------------------------ */
 
 /* Device sincos used by the integrator (csrc/aw_trig.cuh), evaluated on n device doubles. */

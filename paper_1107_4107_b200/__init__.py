@@ -10,7 +10,7 @@ from .binding import (AW_DENS_ACTION, AW_DENS_VEL_BOTH, AW_DENS_VEL_LOWER, AW_DE
                       AW_IND_VZ, AW_SHAPE_DISK, AW_SHAPE_GAUSS, AW_SHAPE_GRID, AW_SHAPE_SPHERE,
                       AW_ST_LEFT, AW_ST_LIVE, AW_ST_NONFINITE, AW_ST_OFFSHELL, AwError, Ensemble, Grid,
                       aw_common_tangent, aw_density, aw_energy_stats, aw_energy_stats_scratch_bytes, aw_dfma_peak_probe, aw_dfma_shape_probe, aw_hamiltonian_probe,
-                      aw_indicator, aw_init_shell, aw_integrate, aw_launch_count, aw_map_host, aw_mark,
+                      aw_indicator, aw_init_shell, aw_integrate, aw_launch_count, aw_map_host, aw_mark, aw_velocity_map_host,
                       aw_sincos_probe, aw_stage_constants, aw_state_bytes, aw_strerror,
                       aw_trig_level, aw_uniform_probe, aw_version, lib, make_grid)
 from .configs import CONFIGS

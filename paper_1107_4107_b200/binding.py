@@ -97,6 +97,8 @@ def lib():
         L.aw_trig_level.argtypes = [C.POINTER(AwState), dbl]
         L.aw_map_host.argtypes = [C.POINTER(AwState), C.POINTER(HostIn), i64, dbl, i64, C.c_int, dbl,
                                   i32, i32, dbl, dbl, vp, vp, C.POINTER(HostOut)]
+        L.aw_velocity_map_host.argtypes = [C.POINTER(AwState), C.POINTER(HostIn), i64, dbl, i64, C.c_int, i32, i32,
+                                           dbl, dbl, vp, C.POINTER(HostOut)]
         L.aw_sincos_probe.argtypes = [vp, i64, vp, vp, vp]
         L.aw_uniform_probe.argtypes = [u64, u64, i64, C.c_uint32, vp, vp]
         L.aw_hamiltonian_probe.argtypes = [vp, i64, i64, dbl, vp, vp]
@@ -292,6 +294,18 @@ def aw_map_host(ens, host_in, steps, dt, stride, kind, thr, hist_shape, lo, hi, 
     gy, gx = hist_shape
     _check(lib().aw_map_host(C.byref(ens.c), C.byref(hin), steps, dt, stride, kind, thr, gx, gy, lo, hi,
                              _ptr(ind_dev), _ptr(hist_dev), C.byref(hout)), "aw_map_host")
+
+
+def aw_velocity_map_host(ens, host_in, steps, dt, stride, mode, hist_shape, lo, hi, hist_dev, host_out, stream=None):
+    """The paper's pipeline with host buffers: upload, aw_mark, aw_integrate, aw_density(mode 1..3), download."""
+    ens.bind_stream(stream)
+    hin = HostIn(_ptr(host_in["q"]), _ptr(host_in.get("w")), _ptr(host_in["acc"]),
+                 _ptr(host_in.get("wind")), _ptr(host_in["status"]))
+    hout = HostOut(None, _ptr(host_out.get("hist")), _ptr(host_out.get("dropped")),
+                   _ptr(host_out.get("q")), _ptr(host_out.get("acc")), _ptr(host_out.get("status")))
+    gy, gx = hist_shape
+    _check(lib().aw_velocity_map_host(C.byref(ens.c), C.byref(hin), steps, dt, stride, mode, gx, gy, lo, hi,
+                                      _ptr(hist_dev), C.byref(hout)), "aw_velocity_map_host")
 
 
 # ------------------------------------------------------------------------------ probes

@@ -461,6 +461,40 @@ int aw_map_host(aw_state *s, const aw_host_in *in, int64_t steps, double dt, int
   return AW_OK;
 }
 
+int aw_velocity_map_host(aw_state *s, const aw_host_in *in, int64_t steps, double dt, int64_t stride, int mode,
+                         int32_t gx, int32_t gy, double lo, double hi, void *hist_dev, const aw_host_out *out) {
+  if (!s || !in || !out || !hist_dev || !out->hist) return AW_EINVAL;
+  int rc = check_planes(s);
+  if (rc != AW_OK) return rc;
+  if (!in->q || !in->acc || !in->status || (s->w && !in->w) || (s->wind && !in->wind)) return AW_EINVAL;
+  if (mode < AW_DENS_VEL_UPPER || mode > AW_DENS_VEL_BOTH || gx <= 0 || gy <= 0) return AW_EINVAL;
+  if (s->n > 0 && !has_ref(s)) return AW_ESTATE;
+  cudaStream_t st = (cudaStream_t)s->stream;
+  const size_t P = (size_t)s->pitch;
+  AW_CUDA(cudaMemcpyAsync(s->q, in->q, 6 * P * 8, cudaMemcpyHostToDevice, st));
+  if (s->w) AW_CUDA(cudaMemcpyAsync(s->w, in->w, 6 * P * 8, cudaMemcpyHostToDevice, st));
+  AW_CUDA(cudaMemcpyAsync(s->acc, in->acc, 4 * P * 8, cudaMemcpyHostToDevice, st));
+  if (s->wind) AW_CUDA(cudaMemcpyAsync(s->wind, in->wind, 3 * P * 4, cudaMemcpyHostToDevice, st));
+  AW_CUDA(cudaMemcpyAsync(s->status, in->status, (size_t)s->n, cudaMemcpyHostToDevice, st));
+  s->ready = 1;
+  rc = aw_mark(s);
+  if (rc != AW_OK) return rc;
+  rc = aw_integrate(s, s->n, steps, dt, stride);
+  if (rc != AW_OK) return rc;
+  const size_t hb = (size_t)gx * gy * 4;
+  AW_CUDA(cudaMemsetAsync(hist_dev, 0, hb + 8, st));
+  uint64_t *drop_dev = reinterpret_cast<uint64_t *>(static_cast<char *>(hist_dev) + hb);
+  rc = aw_density(s, static_cast<uint32_t *>(hist_dev), gx, gy, lo, hi, mode, drop_dev);
+  if (rc != AW_OK) return rc;
+  AW_CUDA(cudaMemcpyAsync(out->hist, hist_dev, hb, cudaMemcpyDeviceToHost, st));
+  if (out->dropped) AW_CUDA(cudaMemcpyAsync(out->dropped, drop_dev, 8, cudaMemcpyDeviceToHost, st));
+  if (out->q) AW_CUDA(cudaMemcpyAsync(out->q, s->q, 6 * P * 8, cudaMemcpyDeviceToHost, st));
+  if (out->acc) AW_CUDA(cudaMemcpyAsync(out->acc, s->acc, 4 * P * 8, cudaMemcpyDeviceToHost, st));
+  if (out->status) AW_CUDA(cudaMemcpyAsync(out->status, s->status, (size_t)s->n, cudaMemcpyDeviceToHost, st));
+  AW_CUDA(cudaStreamSynchronize(st));
+  return AW_OK;
+}
+
 int aw_sincos_probe(const double *x_dev, int64_t n, double *sin_dev, double *cos_dev, void *stream) {
   if (!x_dev || !sin_dev || !cos_dev || n < 0) return AW_EINVAL;
   if (n == 0) return AW_OK;

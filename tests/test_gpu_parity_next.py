@@ -545,3 +545,41 @@ def test_gpu_velocity_closed_forms(aw, order):
     tol = 1e-8 if order == 4 else 1e-10
     assert np.max(np.abs(X / (5 * T) - 2 * math.pi / T)) < tol
     assert np.all(qf[[1, 2, 4, 5], :32] == 0.0)               # the invariant subspace, exactly
+
+
+def test_velocity_map_host_equals_the_device_path(aw, orc):
+    """aw_velocity_map_host (host buffers in, sphere density out) = upload + aw_mark + aw_integrate + aw_density
+    on the device, bit for bit, and the histogram equals the oracle's binning of the returned state."""
+    cfg = aw.CONFIGS[6]
+    gx, gy = 96, 40
+    n = gx * gy
+    R = math.sqrt(2 * cfg["E"])
+    a = aw.Ensemble(n, tangent=False, wind=True, order=6, ref=True)
+    aw.aw_init_shell(a, aw.make_grid(gx, gy, angle_mode=1, shape=aw.AW_SHAPE_SPHERE), cfg["E"], cfg["eps"], 6)
+    host_in = dict(q=a.q.cpu().pin_memory(), acc=a.acc.cpu().pin_memory(), wind=a.wind.cpu().pin_memory(),
+                   status=a.status[:n].cpu().pin_memory())
+    aw.aw_mark(a)
+    aw.aw_integrate(a, n, 1000, cfg["dt"], 100)
+    hist = torch.zeros((128, 128), dtype=torch.int32, device="cuda")
+    dropped = torch.zeros(1, dtype=torch.int64, device="cuda")
+    aw.aw_density(a, hist, -R, R, aw.AW_DENS_VEL_UPPER, dropped)
+    b = aw.Ensemble(n, tangent=False, wind=True, order=6, ref=True)
+    b.c.E, b.c.eps = cfg["E"], cfg["eps"]
+    out = dict(hist=torch.empty((128, 128), dtype=torch.int32).pin_memory(),
+               dropped=torch.zeros(1, dtype=torch.int64).pin_memory(),
+               q=torch.empty((6, b.pitch), dtype=torch.float64).pin_memory())
+    hist_dev = torch.empty(128 * 128 + 2, dtype=torch.int32, device="cuda")
+    aw.aw_velocity_map_host(b, host_in, 1000, cfg["dt"], 100, aw.AW_DENS_VEL_UPPER, (128, 128), -R, R, hist_dev, out)
+    assert torch.equal(out["hist"], hist.cpu()) and out["dropped"].item() == dropped.item()
+    assert torch.equal(out["q"], a.q.cpu()) and b.step == 1000 and b.tref == 0.0
+    st = ensemble_to_oracle(b, orc)
+    ref = np.zeros((128, 128), dtype=np.uint32)
+    d = orc.density_velocity(st, ref, -R, R, 1)
+    assert np.array_equal(out["hist"].numpy().view(np.uint32), ref) and int(d[0]) == out["dropped"].item()
+    assert int(ref.sum()) + int(d[0]) == n and ref.sum() > 0.4 * n
+    # without snapshot planes the call is refused before anything is copied
+    c = aw.Ensemble(n, tangent=False, wind=True, order=6)
+    c.c.E, c.c.eps = cfg["E"], cfg["eps"]
+    with pytest.raises(aw.AwError) as ei:
+        aw.aw_velocity_map_host(c, host_in, 100, cfg["dt"], 100, 1, (128, 128), -R, R, hist_dev, out)
+    assert ei.value.code == -4
