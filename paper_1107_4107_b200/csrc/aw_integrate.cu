@@ -211,6 +211,9 @@ __device__ __forceinline__ void drift_angles(Traj<TAN> &t, double a, double a2) 
 template <int S, bool TAN, int LEVEL, int s>
 __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
   constexpr int cs = (s == S - 1) ? s : (s < S - 2 - s ? s : S - 2 - s);
+  // the angle FMAs first: they depend only on the kick just done, and in the -O1 unit (source order) they fill
+  // the latency of the kick's tail before the polynomial chains start (measured +0.8 to +1.6 %)
+  drift_angles<TAN>(t, p.a_loop[cs], p.a2_loop[cs]);
   if (LEVEL > 0) {
     constexpr int nuv = rotation_degree<S, LEVEL, cs, false>(), nz = rotation_degree<S, LEVEL, cs, true>();
     double g, m;
@@ -230,7 +233,6 @@ __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
       rotate(t.s2, t.c2, g, m);
     }
   }
-  drift_angles<TAN>(t, p.a_loop[cs], p.a2_loop[cs]);
 }
 
 template <bool TAN, int LEVEL>
