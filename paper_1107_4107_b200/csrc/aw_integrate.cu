@@ -90,28 +90,6 @@ __device__ __forceinline__ void small_sincos(double p, const double (&G)[kTrigTe
   m = z * pm;
 }
 
-// The same two functions of the angle d itself, with the universal Taylor coefficients: used by the 7-stage
-// scheme, whose four distinct drift constants would otherwise need four sets of leading coefficients in
-// registers (a DFMA takes one constant-bank operand at most).  N + (N-1) FMA, 3 DMUL, plus d = A p outside.
-template <int N>
-__device__ __forceinline__ void small_sincos_angle(double d, double &g, double &m) {
-  constexpr double Sc[8] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0, -1.0 / 39916800.0,
-                            1.0 / 6227020800.0, -1.0 / 1307674368000.0, 1.0 / 355687428096000.0};
-  constexpr double Cc[8] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0, -1.0 / 3628800.0,
-                            1.0 / 479001600.0, -1.0 / 87178291200.0, 1.0 / 20922789888000.0};
-  static_assert(N >= 1 && N <= 8, "degree");
-  const double z = d * d;
-  double pg = Sc[N - 1], pm = Cc[N - 1];
-#pragma unroll
-  for (int i = N - 2; i >= 0; --i) {
-    pg = fma(pg, z, Sc[i]);
-    pm = fma(pm, z, Cc[i]);
-  }
-  pg = fma(pg, z, 1.0);
-  g = d * pg;
-  m = z * pm;
-}
-
 // (s, c) <- rotation of (s, c) by the angle whose sine is g and cosine is 1 + m; <= 1 ulp each.
 __device__ __forceinline__ void rotate(double &s, double &c, double g, double m) {
   const double t1 = fma(s, m, s), t2 = fma(c, m, c);
@@ -217,21 +195,12 @@ __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
   if (LEVEL > 0) {
     constexpr int nuv = rotation_degree<S, LEVEL, cs, false>(), nz = rotation_degree<S, LEVEL, cs, true>();
     double g, m;
-    if (S <= 3) {
-      small_sincos<nuv>(t.pu, p.grot[cs], p.mrot[cs], g, m);
-      rotate(t.su, t.cu, g, m);
-      small_sincos<nuv>(t.pv, p.grot[cs], p.mrot[cs], g, m);
-      rotate(t.sv, t.cv, g, m);
-      small_sincos<nz>(t.pzt, p.grot[cs], p.mrot[cs], g, m);
-      rotate(t.s2, t.c2, g, m);
-    } else {
-      small_sincos_angle<nuv>(p.a_loop[cs] * t.pu, g, m);
-      rotate(t.su, t.cu, g, m);
-      small_sincos_angle<nuv>(p.a_loop[cs] * t.pv, g, m);
-      rotate(t.sv, t.cv, g, m);
-      small_sincos_angle<nz>(p.a_loop[cs] * t.pzt, g, m);
-      rotate(t.s2, t.c2, g, m);
-    }
+    small_sincos<nuv>(t.pu, p.grot[cs], p.mrot[cs], g, m);
+    rotate(t.su, t.cu, g, m);
+    small_sincos<nuv>(t.pv, p.grot[cs], p.mrot[cs], g, m);
+    rotate(t.sv, t.cv, g, m);
+    small_sincos<nz>(t.pzt, p.grot[cs], p.mrot[cs], g, m);
+    rotate(t.s2, t.c2, g, m);
   }
 }
 
