@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libaw.so")
 SOURCES = ["aw_api.cu", "aw_integrate.cu", "aw_init.cu", "aw_reduce.cu"]
-# (source, object, extra flags): aw_integrate.cu is compiled a second time for the kernels of trig levels 1-4 with
+# (source, object, extra flags): aw_integrate.cu is compiled a second time for the rotation kernels (trig levels 1-7) with
 # ptxas -O1, whose scheduling keeps operand-sharing FMAs adjacent (see the comment at AW_LEVEL_GROUP in the source)
 UNITS = [("aw_api.cu", "aw_api.o", []), ("aw_integrate.cu", "aw_integrate.o", []),
          ("aw_integrate.cu", "aw_integrate_low.o", ["-DAW_LEVEL_GROUP=1", "-Xptxas", "-O1"]),

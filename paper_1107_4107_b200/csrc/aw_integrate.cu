@@ -51,11 +51,12 @@
 #define AW_MIN_BLOCKS(LEVEL) ((LEVEL) == 4 ? 4 : 3)
 #endif
 
-// This file is compiled twice (build.py).  AW_LEVEL_GROUP 1 instantiates the kernels of trig levels 1-4 and is
-// compiled with -Xptxas -O1: ptxas's lighter scheduler keeps the three-register FMAs that share an operand next
-// to each other, so more of them hit the operand-reuse cache (measured on B200: configs[3] +3.5 %, configs[2]
-// +3.5 %, order 6 +2.9 %, configs[4] +1.5 %).  AW_LEVEL_GROUP 0 (default flags) holds levels 0 and 5-7, which
-// lose 2-3 % at -O1, and the host-side functions.
+// This file is compiled twice (build.py).  AW_LEVEL_GROUP 1 instantiates the rotation kernels (trig levels 1-7)
+// and is compiled with -Xptxas -O1: ptxas's lighter scheduler stays close to source order, which keeps the
+// three-register FMAs that share an operand next to each other, so more of them hit the operand-reuse cache
+// (measured on B200: configs[3] +3.5 %, configs[2] +3.5 %, order 6 +2.9 %, configs[4] +1.5 %, level 7 +1.6 %), and
+// needs fewer registers (the 7-stage scheme's four coefficient sets fit).  AW_LEVEL_GROUP 0 (default flags) holds
+// the level-0 kernels (device sincos at every stage), which lose 3 % at -O1, and the host-side functions.
 #ifndef AW_LEVEL_GROUP
 #define AW_LEVEL_GROUP 0
 #endif
@@ -347,11 +348,11 @@ cudaError_t launch_level(const IntegrateParams &p, cudaStream_t st) {
     case 2: return launch_one<S, TAN, 2>(p, st);
     case 3: return launch_one<S, TAN, 3>(p, st);
     case 4: return launch_one<S, TAN, 4>(p, st);
-    default: return cudaErrorInvalidValue;
-#else
     case 5: return launch_one<S, TAN, 5>(p, st);
     case 6: return launch_one<S, TAN, 6>(p, st);
     case 7: return launch_one<S, TAN, 7>(p, st);
+    default: return cudaErrorInvalidValue;
+#else
     default: return launch_one<S, TAN, 0>(p, st);
 #endif
   }
@@ -398,7 +399,7 @@ bool drift_ratios_hold(int S, const double *a_loop) {
 cudaError_t launch_integrate_low(const IntegrateParams &p, int order, bool tangent, cudaStream_t st);
 
 cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, cudaStream_t st) {
-  if (p.level >= 1 && p.level <= 4) return launch_integrate_low(p, order, tangent, st);
+  if (p.level >= 1) return launch_integrate_low(p, order, tangent, st);
   if (order == 4) return tangent ? launch_level<3, true>(p, st) : launch_level<3, false>(p, st);
   return tangent ? launch_level<7, true>(p, st) : launch_level<7, false>(p, st);
 }
