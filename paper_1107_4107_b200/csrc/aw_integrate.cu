@@ -56,7 +56,8 @@
 // three-register FMAs that share an operand next to each other, so more of them hit the operand-reuse cache
 // (measured on B200: configs[3] +3.5 %, configs[2] +3.5 %, order 6 +2.9 %, configs[4] +1.5 %, level 7 +1.6 %), and
 // needs fewer registers (the 7-stage scheme's four coefficient sets fit).  AW_LEVEL_GROUP 0 (default flags) holds
-// the level-0 kernels (device sincos at every stage), which lose 3 % at -O1, and the host-side functions.
+// the kernels that evaluate the device sincos in the step loop (level 0: at every stage; the mixed level 8), which
+// lose 2-3 % at -O1, and the host-side functions.
 #ifndef AW_LEVEL_GROUP
 #define AW_LEVEL_GROUP 0
 #endif
@@ -108,7 +109,11 @@ __device__ __forceinline__ void rotate(double &s, double &c, double g, double m)
 //   N = 1: t <= 6.8e-5;  2: 0.00293;  3: 0.0208;  4: 0.0708;  5: 0.165;  6: 0.310;  7: 0.505;  8: 0.750.
 // The largest drift (the merged one) gets degrees (3,3), (3,4), (4,4), (4,5), (5,6), (6,7), (7,8) at levels
 // 1..7; the short inner drifts of the triple jump (ratio 0.13) and of the 7-stage scheme (0.088) one or two less.
-constexpr double kLevelMaxD[8] = {0.0, 0.0104, 0.0147, 0.0354, 0.0500, 0.1166, 0.2192, 0.3570};
+// Level 8 (|d| <= 2) is mixed: a drift whose own largest angle still fits degree <= 8 rotates the pairs, the
+// others leave them stale and the kick that follows evaluates the device sincos instead (degree 0 below): with
+// the triple jump two of three stages rotate, with the 7-stage scheme two of seven (its 0.088 drifts).  Every
+// step contains a sincos stage (the merged drift never rotates there), so level 8 needs no re-synchronisation.
+constexpr double kLevelMaxD[9] = {0.0, 0.0104, 0.0147, 0.0354, 0.0500, 0.1166, 0.2192, 0.3570, 2.0};
 constexpr double kDegreeMaxAngle[9] = {0.0, 6.8e-5, 0.00293, 0.0208, 0.0708, 0.165, 0.310, 0.505, 0.750};
 
 // upper bounds of |a_loop[cs]| / max_s |a_loop[s]| for the coefficient sets cs of drift() (cs = S-1: merged drift)
@@ -118,11 +123,18 @@ template <> struct DriftRatio<7> { static constexpr double r[7] = {0.6502, 0.600
 
 template <int S, int LEVEL, int cs, bool ZETA>
 __host__ __device__ constexpr int rotation_degree() {
-  if (LEVEL == 0) return 1;  // unused
+  if (LEVEL == 0) return 0;  // no rotation: device sincos at every stage
   const double t = (ZETA ? 2.0 : 1.4142135623730951) * kLevelMaxD[LEVEL] * DriftRatio<S>::r[cs];
   int n = 1;
   while (n < 8 && kDegreeMaxAngle[n] < t) ++n;
-  return n;
+  return kDegreeMaxAngle[n] < t ? 0 : n;  // 0: the angle is too large for a degree-8 rotation
+}
+
+// does the drift after kick s rotate the running pairs (true at levels 1-7, per drift at level 8, never at 0)?
+template <int S, int LEVEL, int s>
+__host__ __device__ constexpr bool drift_rotates() {
+  constexpr int cs = (s == S - 1) ? s : (s < S - 2 - s ? s : S - 2 - s);
+  return rotation_degree<S, LEVEL, cs, false>() > 0 && rotation_degree<S, LEVEL, cs, true>() > 0;
 }
 
 // Everything a thread carries between stages.  Inside a block of `stride` steps the state is held in the
@@ -193,7 +205,7 @@ __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
   // the angle FMAs first: they depend only on the kick just done, and in the -O1 unit (source order) they fill
   // the latency of the kick's tail before the polynomial chains start (measured +0.8 to +1.6 %)
   drift_angles<TAN>(t, p.a_loop[cs], p.a2_loop[cs]);
-  if (LEVEL > 0) {
+  if constexpr (drift_rotates<S, LEVEL, s>()) {
     constexpr int nuv = rotation_degree<S, LEVEL, cs, false>(), nz = rotation_degree<S, LEVEL, cs, true>();
     double g, m;
     small_sincos<nuv>(t.pu, p.grot[cs], p.mrot[cs], g, m);
@@ -207,7 +219,7 @@ __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
 
 template <bool TAN, int LEVEL>
 __device__ __forceinline__ void resync(Traj<TAN> &t) {
-  if (LEVEL > 0) {
+  if (LEVEL > 0 && LEVEL < 8) {
     sincos(t.u, t.su, t.cu);
     sincos(t.v, t.sv, t.cv);
     sincos(t.zt, t.s2, t.c2);
@@ -221,9 +233,10 @@ __device__ __forceinline__ void resync(Traj<TAN> &t) {
 //   dpv += b (F cos v dv - sin zeta sin v dzeta)
 //   dpz += b (-sin zeta (sin u du + sin v dv) + W cos zeta dzeta)
 // (the sum and difference of the x and y rows of SURVEY.md Appendix A.2, with dzeta = 2 dz).
-template <bool TAN, int LEVEL>
+// FRESH: the running pairs are valid (the drift before this kick rotated them); otherwise they are evaluated here.
+template <bool TAN, bool FRESH>
 __device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2) {
-  if (LEVEL == 0) {
+  if (!FRESH) {
     sincos(t.u, t.su, t.cu);
     sincos(t.v, t.sv, t.cv);
     sincos(t.zt, t.s2, t.c2);
@@ -248,7 +261,8 @@ __device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2) {
 template <int S, bool TAN, int LEVEL, int s>
 __device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p) {
   if constexpr (s < S) {
-    kick<TAN, LEVEL>(t, p.b1[s], p.b2[s]);
+    // the drift before kick s is the one after kick s-1, or for s = 0 the merged drift that closed the last step
+    kick<TAN, drift_rotates<S, LEVEL, (s == 0 ? S - 1 : s - 1)>()>(t, p.b1[s], p.b2[s]);
     drift<S, TAN, LEVEL, s>(t, p);
     stages<S, TAN, LEVEL, s + 1>(t, p);
   }
@@ -353,6 +367,7 @@ cudaError_t launch_level(const IntegrateParams &p, cudaStream_t st) {
     case 7: return launch_one<S, TAN, 7>(p, st);
     default: return cudaErrorInvalidValue;
 #else
+    case 8: return launch_one<S, TAN, 8>(p, st);
     default: return launch_one<S, TAN, 0>(p, st);
 #endif
   }
@@ -376,11 +391,12 @@ cudaError_t launch_integrate_low(const IntegrateParams &p, int order, bool tange
 // The u and v pairs rotate by up to sqrt(2) |d|, the 2z pair by up to 2 |d|:
 //   level 1 = (3,3): 2|d| <= 0.0208;       level 2 = (3,4): sqrt(2)|d| <= 0.0208;   level 3 = (4,4): 2|d| <= 0.0708;
 //   level 4 = (4,5): sqrt(2)|d| <= 0.0708;  level 5 = (5,6): sqrt(2)|d| <= 0.165;    level 6 = (6,7): sqrt(2)|d| <= 0.310;
-//   level 7 = (7,8): sqrt(2)|d| <= 0.505 (and 2|d| <= 0.750);  beyond: level 0 (full sincos every stage), which is
-//   also cheaper from there on: a degree-(8,9) rotation costs more fp64 instructions than the sincos it replaces.
+//   level 7 = (7,8): sqrt(2)|d| <= 0.505 (and 2|d| <= 0.750);  level 8 (|d| <= 2): mixed, see kLevelMaxD;
+//   beyond: level 0 (full sincos every stage).  A degree-(8,9) rotation of the merged drift would cost more fp64
+//   instructions than the sincos it replaces, which is why the pure rotation levels stop at 7.
 int trig_level_for(double d) {
   if (!(d == d)) return 0;
-  for (int level = 1; level <= 7; ++level)
+  for (int level = 1; level <= 8; ++level)
     if (d <= kLevelMaxD[level]) return level;
   return 0;
 }
@@ -399,7 +415,7 @@ bool drift_ratios_hold(int S, const double *a_loop) {
 cudaError_t launch_integrate_low(const IntegrateParams &p, int order, bool tangent, cudaStream_t st);
 
 cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, cudaStream_t st) {
-  if (p.level >= 1) return launch_integrate_low(p, order, tangent, st);
+  if (p.level >= 1 && p.level <= 7) return launch_integrate_low(p, order, tangent, st);
   if (order == 4) return tangent ? launch_level<3, true>(p, st) : launch_level<3, false>(p, st);
   return tangent ? launch_level<7, true>(p, st) : launch_level<7, false>(p, st);
 }

@@ -217,12 +217,12 @@ def test_tangent_state_and_fli_parity_short_horizon(aw, orc, order, cfgk):
 
 @pytest.mark.parametrize("order,dt,stride,level", [
     (4, 0.005, 100, 1), (4, 0.007, 100, 2), (4, 0.015, 100, 3), (4, 0.025, 100, 4), (4, 0.05, 100, 5),
-    (4, 0.1, 100, 6), (4, 0.15, 100, 7), (4, 0.2, 100, 0),
+    (4, 0.1, 100, 6), (4, 0.15, 100, 7), (4, 0.2, 100, 8),
     (6, 0.005, 100, 1), (6, 0.012, 100, 2), (6, 0.02, 100, 3), (6, 0.04, 100, 4), (6, 0.08, 100, 5),
     (6, 0.15, 100, 6), (6, 0.25, 100, 7),
     (4, 0.005, 300, 1), (4, 0.007, 1000, 2), (4, 0.007, 7, 2), (6, 0.02, 1, 3), (4, -0.007, 250, 2)])
 def test_every_trig_level_matches_the_oracle(aw, orc, order, dt, stride, level):
-    """The running-(sin, cos) variants (levels 1-7: Taylor degrees picked from the largest drift angle,
+    """The running-(sin, cos) variants (levels 1-7 and the mixed level 8: Taylor degrees picked from the largest drift angle,
     re-synchronised every checkpoint and every <= 128 steps) and the full-sincos variant (level 0, also
     forced with trig = 1) all reproduce the oracle within the state tolerance; seeded random angles,
     eps = 3e-2, tangent map on; strides that split into several re-synchronisation chunks and stride 1."""
