@@ -155,8 +155,8 @@ AW_API int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps,
  * max_s |a_s| sqrt(2(E + 2|eps|)) so the truncation stays below 2^-60; aw_trig_level reports it), and
  * recomputes them from the angles with the device sincos at every checkpoint and at least every 128
  * steps.  s->E must therefore bound the energy of an uploaded state.  If the drift angle can exceed
- * 0.357 rad the kernel is mixed (level 8, up to 2 rad): the scheme's short drifts still rotate the pairs, the long
- * ones are followed by the device sincos; beyond 2 rad, or with s->trig == 1, the device sincos is evaluated at
+ * 0.357 rad the kernel is mixed (levels 8 and 9, up to 0.54 and 2 rad): the scheme's shorter drifts still rotate the
+ * pairs, the long ones are followed by the device sincos; beyond 2 rad, or with s->trig == 1, the device sincos is evaluated at
  * every stage (level 0).
  * The work is split into kernel launches of at most AW_MAX_STEPS_PER_LAUNCH steps (a multiple of
  * stride); the result does not depend on the split. */
@@ -215,7 +215,7 @@ AW_API int aw_density(const aw_state *s, uint32_t *hist_dev, int32_t gx, int32_t
 AW_API int aw_stage_constants(int order, double dt, double eps, double *a_host, double *b_host);
 /* Trigonometry level aw_integrate would use for this state and dt: 0 = device sincos at every stage,
  * 1..7 = running pairs with Taylor degrees (x+y / x-y pairs, 2z pair) = (3,3), (3,4), (4,4), (4,5), (5,6),
- * (6,7), (7,8), 8 = mixed (rotations through the short drifts, device sincos after the long ones); or a
+ * (6,7), (7,8), 8 and 9 = mixed (rotations through the shorter drifts, device sincos after the long ones); or a
  * negative aw_status.  Pure host arithmetic. */
 AW_API int aw_trig_level(const aw_state *s, double dt);
 /* The common tangent vector of tangent_mode 0: unit vector from u(seed, 2^63-1, 5..10) (R12). */

@@ -56,7 +56,7 @@
 // three-register FMAs that share an operand next to each other, so more of them hit the operand-reuse cache
 // (measured on B200: configs[3] +3.5 %, configs[2] +3.5 %, order 6 +2.9 %, configs[4] +1.5 %, level 7 +1.6 %), and
 // needs fewer registers (the 7-stage scheme's four coefficient sets fit).  AW_LEVEL_GROUP 0 (default flags) holds
-// the kernels that evaluate the device sincos in the step loop (level 0: at every stage; the mixed level 8), which
+// the kernels that evaluate the device sincos in the step loop (level 0: at every stage; the mixed levels 8, 9), which
 // lose 2-3 % at -O1, and the host-side functions.
 #ifndef AW_LEVEL_GROUP
 #define AW_LEVEL_GROUP 0
@@ -109,11 +109,12 @@ __device__ __forceinline__ void rotate(double &s, double &c, double g, double m)
 //   N = 1: t <= 6.8e-5;  2: 0.00293;  3: 0.0208;  4: 0.0708;  5: 0.165;  6: 0.310;  7: 0.505;  8: 0.750.
 // The largest drift (the merged one) gets degrees (3,3), (3,4), (4,4), (4,5), (5,6), (6,7), (7,8) at levels
 // 1..7; the short inner drifts of the triple jump (ratio 0.13) and of the 7-stage scheme (0.088) one or two less.
-// Level 8 (|d| <= 2) is mixed: a drift whose own largest angle still fits degree <= 8 rotates the pairs, the
-// others leave them stale and the kick that follows evaluates the device sincos instead (degree 0 below): with
-// the triple jump two of three stages rotate, with the 7-stage scheme two of seven (its 0.088 drifts).  Every
-// step contains a sincos stage (the merged drift never rotates there), so level 8 needs no re-synchronisation.
-constexpr double kLevelMaxD[9] = {0.0, 0.0104, 0.0147, 0.0354, 0.0500, 0.1166, 0.2192, 0.3570, 2.0};
+// Levels 8 (|d| <= 0.54) and 9 (|d| <= 2) are mixed: a drift whose own largest angle still fits degree <= 8 rotates
+// the pairs, the others leave them stale and the kick that follows evaluates the device sincos instead (degree 0
+// below).  Level 8: the inner drifts of the triple jump (two of three stages) and all six inner drifts of the
+// 7-stage scheme rotate; level 9: the triple jump's two, and the 7-stage scheme's two 0.088 drifts.  Every step
+// contains a sincos stage (the merged drift never rotates there), so these levels need no re-synchronisation.
+constexpr double kLevelMaxD[10] = {0.0, 0.0104, 0.0147, 0.0354, 0.0500, 0.1166, 0.2192, 0.3570, 0.5400, 2.0};
 constexpr double kDegreeMaxAngle[9] = {0.0, 6.8e-5, 0.00293, 0.0208, 0.0708, 0.165, 0.310, 0.505, 0.750};
 
 // upper bounds of |a_loop[cs]| / max_s |a_loop[s]| for the coefficient sets cs of drift() (cs = S-1: merged drift)
@@ -219,7 +220,7 @@ __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
 
 template <bool TAN, int LEVEL>
 __device__ __forceinline__ void resync(Traj<TAN> &t) {
-  if (LEVEL > 0 && LEVEL < 8) {
+  if (LEVEL > 0 && LEVEL < 8) {  // levels 8, 9 recompute the pairs with the device sincos in every step
     sincos(t.u, t.su, t.cu);
     sincos(t.v, t.sv, t.cv);
     sincos(t.zt, t.s2, t.c2);
@@ -368,6 +369,7 @@ cudaError_t launch_level(const IntegrateParams &p, cudaStream_t st) {
     default: return cudaErrorInvalidValue;
 #else
     case 8: return launch_one<S, TAN, 8>(p, st);
+    case 9: return launch_one<S, TAN, 9>(p, st);
     default: return launch_one<S, TAN, 0>(p, st);
 #endif
   }
@@ -391,12 +393,12 @@ cudaError_t launch_integrate_low(const IntegrateParams &p, int order, bool tange
 // The u and v pairs rotate by up to sqrt(2) |d|, the 2z pair by up to 2 |d|:
 //   level 1 = (3,3): 2|d| <= 0.0208;       level 2 = (3,4): sqrt(2)|d| <= 0.0208;   level 3 = (4,4): 2|d| <= 0.0708;
 //   level 4 = (4,5): sqrt(2)|d| <= 0.0708;  level 5 = (5,6): sqrt(2)|d| <= 0.165;    level 6 = (6,7): sqrt(2)|d| <= 0.310;
-//   level 7 = (7,8): sqrt(2)|d| <= 0.505 (and 2|d| <= 0.750);  level 8 (|d| <= 2): mixed, see kLevelMaxD;
+//   level 7 = (7,8): sqrt(2)|d| <= 0.505 (and 2|d| <= 0.750);  levels 8 (|d| <= 0.54) and 9 (|d| <= 2): mixed, see kLevelMaxD;
 //   beyond: level 0 (full sincos every stage).  A degree-(8,9) rotation of the merged drift would cost more fp64
 //   instructions than the sincos it replaces, which is why the pure rotation levels stop at 7.
 int trig_level_for(double d) {
   if (!(d == d)) return 0;
-  for (int level = 1; level <= 8; ++level)
+  for (int level = 1; level <= 9; ++level)
     if (d <= kLevelMaxD[level]) return level;
   return 0;
 }

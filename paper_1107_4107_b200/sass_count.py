@@ -82,5 +82,5 @@ def integrate_step_mix(order, tangent, level, lib=LIB):
 if __name__ == "__main__":
     for order in (4, 6):
         for tangent in (False, True):
-            for level in range(9):
+            for level in range(10):
                 print(order, tangent, level, integrate_step_mix(order, tangent, level))

@@ -105,11 +105,11 @@ def test_validation_happens_on_the_host(aw):
     st.q = base
     # trigonometry level picked on the host from the largest drift angle (include/aw.h, aw_integrate)
     lv = lambda dt: L.aw_trig_level(C.byref(st), dt)
-    assert [lv(0.005), lv(-0.005), lv(0.007), lv(0.01), lv(0.02), lv(0.03), lv(0.1), lv(0.15), lv(0.5), lv(1.2)] == \
-        [1, 1, 2, 3, 4, 5, 6, 7, 8, 0]
+    assert [lv(0.005), lv(-0.005), lv(0.007), lv(0.01), lv(0.02), lv(0.03), lv(0.1), lv(0.15), lv(0.2), lv(0.5),
+            lv(1.2)] == [1, 1, 2, 3, 4, 5, 6, 7, 8, 9, 0]
     st.order = 6                                      # largest |c_s| is 0.7845 instead of 1.3512
-    assert [lv(0.005), lv(0.01), lv(0.02), lv(0.04), lv(0.05), lv(0.15), lv(0.3), lv(0.4), lv(2.0)] == \
-        [1, 2, 3, 4, 5, 6, 7, 8, 0]
+    assert [lv(0.005), lv(0.01), lv(0.02), lv(0.04), lv(0.05), lv(0.15), lv(0.3), lv(0.4), lv(1.0), lv(2.0)] == \
+        [1, 2, 3, 4, 5, 6, 7, 8, 9, 0]
     st.order, st.trig = 4, 1
     assert lv(0.005) == 0
     st.trig = 0

@@ -141,7 +141,7 @@ def test_velocity_parity_of_independent_runs(aw, orc):
 def test_paper_units_pipeline_parity(aw, orc, E):
     """eps = 1, E = 15 / 400, sixth-order scheme, h = 0.01 T (T = 2 pi), ICs uniform on
     S x torus, averaging window Dt = 50 T = 5000 steps.  Drift angles reach ~1.4 rad per stage at E = 400, so the
-    kernel is the mixed level 8 (device sincos at five of the seven stages, rotations through the two short
+    kernel is the mixed level 9 (device sincos at five of the seven stages, rotations through the two short
     drifts); at E = 15 (0.29 rad) it is the highest pure rotation level, degrees (7, 8).  State parity after 100 steps (these
     energies are chaotic over much of the sphere: the short north_star horizon applies to everyone), then
     the full window on the GPU and the sphere density bit-exact on the device states."""
@@ -150,7 +150,7 @@ def test_paper_units_pipeline_parity(aw, orc, E):
     n = gx * gy
     ens = aw.Ensemble(n, tangent=False, wind=True, order=6, ref=True)
     aw.aw_init_shell(ens, aw.make_grid(gx, gy, angle_mode=1, shape=aw.AW_SHAPE_SPHERE), E, 1.0, 2011)
-    assert aw.aw_trig_level(ens, h) == (7 if E == 15.0 else 8)
+    assert aw.aw_trig_level(ens, h) == (7 if E == 15.0 else 9)
     aw.aw_mark(ens)
     st = ensemble_to_oracle(ens, orc)
     aw.aw_integrate(ens, n, 100, h, 100)
@@ -585,10 +585,10 @@ def test_velocity_map_host_equals_the_device_path(aw, orc):
     assert ei.value.code == -4
 
 
-@pytest.mark.parametrize("order,dt", [(6, 0.4), (6, 1.2), (4, 0.5), (4, 0.9)])
-def test_mixed_trig_level_8_parity(aw, orc, order, dt):
-    """Level 8 (drift angles up to 2 rad): the short drifts of each scheme rotate the running pairs, the long
-    ones are followed by the device sincos.  Tangent map on, seeded angles, eps = 3e-2, 200 steps (t up to 240:
+@pytest.mark.parametrize("order,dt,level", [(6, 0.4, 8), (6, 1.2, 9), (4, 0.25, 8), (4, 0.5, 9), (4, 0.9, 9)])
+def test_mixed_trig_levels_parity(aw, orc, order, dt, level):
+    """Levels 8 and 9 (drift angles up to 0.54 and 2 rad): the shorter drifts of each scheme rotate the running pairs,
+    the long ones are followed by the device sincos.  Tangent map on, seeded angles, eps = 3e-2, 200 steps (t up to 240:
     the horizon is kept short because at these step sizes the tangent vector shears quickly), against the
     oracle and against the forced level-0 kernel."""
     cfg = dict(aw.CONFIGS[3])
@@ -599,7 +599,7 @@ def test_mixed_trig_level_8_parity(aw, orc, order, dt):
         ens = aw.Ensemble(n, tangent=True, wind=True, order=order)
         aw.aw_init_shell(ens, aw.make_grid(gx, gy, -1.0, 1.0, angle_mode=1), 1.0, cfg["eps"], 5)
         ens.trig = trig
-        assert aw.aw_trig_level(ens, dt) == (0 if trig else 8)
+        assert aw.aw_trig_level(ens, dt) == (0 if trig else level)
         if trig == 0:
             st = ensemble_to_oracle(ens, orc)
         aw.aw_integrate(ens, n, 200, dt, 50)
