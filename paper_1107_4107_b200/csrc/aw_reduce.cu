@@ -228,6 +228,12 @@ __global__ void __launch_bounds__(kDensityBlock)
       if (!in) ++my_dropped;
     }
     const unsigned peers = __match_any_sync(0xffffffffu, bin);
+    // spread input: when no two lanes of the warp share a bin the block table would only add a shared-memory
+    // round trip in front of the same global atomic, so the points go straight to the histogram
+    if (__all_sync(0xffffffffu, bin == kEmpty || __popc(peers) == 1)) {
+      if (bin != kEmpty) atomicAdd(&hist[bin], 1u);
+      continue;
+    }
     if (bin != kEmpty && (__ffs(peers) - 1) == (int)(threadIdx.x & 31)) {
       const unsigned cnt = __popc(peers);
       unsigned slot = (bin * 2654435761u) >> 21;  // top 11 bits -> [0, 2048)
