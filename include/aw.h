@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define AW_VERSION 110 /* 1.1.0 */
+#define AW_VERSION 120 /* 1.2.0 */
 
 #if defined(__GNUC__)
 #define AW_API __attribute__((visibility("default")))
