@@ -260,6 +260,8 @@ struct awo_grid {
   double cx, cy, r;
   int32_t pz_sign;       // +1 or -1
   int32_t tangent_mode;  // 0: one common seeded unit vector; 1: per trajectory
+  int64_t k0;            // the state holds trajectories [k0, k0 + n) of the gx*gy ensemble the grid describes
+                         // (independent realisations, so any contiguous slice can be generated alone)
 };
 
 double awo_hp(double x, double y, double z) { return Hp(x, y, z); }
@@ -292,21 +294,24 @@ int awo_checkpoint(double *q, double *tw, double *acc, int32_t *wind, double eps
 // SoA planes: q[6*pitch], w[6*pitch] or NULL, acc[4*pitch], wind[3*pitch] or NULL, status[n].
 int awo_init_shell(const awo_grid *g, double E, double eps, uint64_t seed, int64_t n, int64_t pitch,
                    double *q, double *w, double *acc, int32_t *wind, uint8_t *status) {
-  if (!g || !q || !acc || !status || n != (int64_t)g->gx * g->gy || pitch < n) return -1;
+  if (!g || !q || !acc || !status || pitch < n) return -1;
+  if (g->k0 < 0 || n < 0 || g->k0 + n > (int64_t)g->gx * g->gy) return -1;
   double tcommon[6];
   unit_tangent(seed, 0x7FFFFFFFFFFFFFFFull, tcommon);
   const double nan = std::numeric_limits<double>::quiet_NaN();
   for (int64_t k = 0; k < n; ++k) {
-    const int64_t i = k % g->gx, j = k / g->gx;
+    // K: index in the whole ensemble (grid position and random-number counter); k: slot in this state's planes
+    const int64_t K = g->k0 + k;
+    const int64_t i = K % g->gx, j = K / g->gx;
     double X[3] = {0.0, 0.0, 0.0};
     if (g->angle_mode == 1)
-      for (int al = 0; al < 3; ++al) X[al] = TWO_PI_HI * uniform01(seed, (uint64_t)k, (uint64_t)al);
+      for (int al = 0; al < 3; ++al) X[al] = TWO_PI_HI * uniform01(seed, (uint64_t)K, (uint64_t)al);
     double st[6];
     if (g->shape == 3) {
       // P:85 "initial conditions uniformly distributed over the sphere S": direction uniform on the unit
       // sphere (cos(theta) = 1 - 2 u3 uniform in (-1, 1], phi = 2 pi u4), |P| from the energy condition
       // H = E: |P|^2 = 2 (E - eps H_p(X)) > 0 always (E > 2|eps|), so no point is off the shell (R28).
-      const double u1 = uniform01(seed, (uint64_t)k, 3), u2 = uniform01(seed, (uint64_t)k, 4);
+      const double u1 = uniform01(seed, (uint64_t)K, 3), u2 = uniform01(seed, (uint64_t)K, 4);
       const double ct = 1.0 - 2.0 * u1;
       const double sth = std::sqrt((1.0 - ct) * (1.0 + ct));
       const double ang = TWO_PI_HI * u2;
@@ -322,7 +327,7 @@ int awo_init_shell(const awo_grid *g, double E, double eps, uint64_t seed, int64
         px = g->lo_x + ((double)i + 0.5) * (g->hi_x - g->lo_x) / (double)g->gx;
         py = g->lo_y + ((double)j + 0.5) * (g->hi_y - g->lo_y) / (double)g->gy;
       } else {
-        const double u1 = uniform01(seed, (uint64_t)k, 3), u2 = uniform01(seed, (uint64_t)k, 4);
+        const double u1 = uniform01(seed, (uint64_t)K, 3), u2 = uniform01(seed, (uint64_t)K, 4);
         const double ang = TWO_PI_HI * u2;
         const double rad = (g->shape == 1) ? g->r * std::sqrt(u1)
                                            : g->r * std::sqrt(-2.0 * std::log(1.0 - u1));
@@ -350,7 +355,7 @@ int awo_init_shell(const awo_grid *g, double E, double eps, uint64_t seed, int64
     acc[3 * pitch + k] = 0.0;                                          // dH_max
     if (w) {
       double t[6];
-      if (g->tangent_mode == 1) unit_tangent(seed, (uint64_t)k, t);
+      if (g->tangent_mode == 1) unit_tangent(seed, (uint64_t)K, t);
       else std::memcpy(t, tcommon, sizeof t);
       for (int c = 0; c < 6; ++c) w[c * pitch + k] = t[c];
     }

@@ -221,7 +221,7 @@ def test_tangent_state_and_fli_parity_short_horizon(aw, orc, order, cfgk):
     (6, 0.005, 100, 1), (6, 0.012, 100, 2), (6, 0.02, 100, 3), (6, 0.04, 100, 4), (6, 0.08, 100, 5),
     (6, 0.15, 100, 6), (6, 0.25, 100, 7),
     (4, 0.005, 300, 1), (4, 0.007, 1000, 2), (4, 0.007, 7, 2), (6, 0.02, 1, 3), (4, -0.007, 250, 2)])
-def test_every_trig_level_matches_the_oracle(aw, orc, order, dt, stride, level):
+def test_every_trig_level_matches_the_oracle(aw, orc, orc_rounding_variant, order, dt, stride, level):
     """The running-(sin, cos) variants (levels 1-7 and the mixed level 8: Taylor degrees picked from the largest drift angle,
     re-synchronised every checkpoint and every <= 128 steps) and the full-sincos variant (level 0, also
     forced with trig = 1) all reproduce the oracle within the state tolerance; seeded random angles,
@@ -236,8 +236,12 @@ def test_every_trig_level_matches_the_oracle(aw, orc, order, dt, stride, level):
         aw.aw_integrate(ens, ens.n, steps, dt, stride)
         res[trig] = ensemble_to_oracle(ens, orc)
     n = st.n
+    st_var = st.copy()
     oracle_integrate_mt(orc, st, steps, dt, stride)
+    oracle_integrate_mt(orc_rounding_variant, st_var, steps, dt, stride)
     live = st.status == 1
+    noise = float(np.max(np.abs(st_var.acc[3, :n][live] - st.acc[3, :n][live])))
+    print("oracle-only rounding noise of dH_max: %.1f ulp(E)" % (noise / (ULP1 * cfg["E"])))
     thr = math.log(st.t) + 3.0
     regular = live & (st.acc[1, :n] <= thr)
     assert regular.sum() > 0.8 * live.sum()
@@ -249,19 +253,15 @@ def test_every_trig_level_matches_the_oracle(aw, orc, order, dt, stride, level):
         assert werr.max() <= 1e-9, (trig, werr.max())
         lo10 = live & (st.acc[1, :n] < 10)
         assert np.max(np.abs(got.acc[1, :n][lo10] - st.acc[1, :n][lo10])) <= 1e-5
-        # dH_max: 64 ulp(E) + 1 % as elsewhere, the absolute part scaled by the size the angles reach
-        # between wraps: an angle of magnitude X carries a rounding error of ulp(X)/2 per drift, which
-        # moves H by eps |grad H_p| ulp(X)/2; at stride |dt| |p| = 7 rad (dt = 0.05) that random walk is
-        # 3x the one at |X| <= pi and is the same for the oracle-vs-oracle-with-FMA comparison
-        # (measured: level 0 and level 4 both differ from the oracle by <= 2.6e-14 there).
-        # dH_max is the largest of steps/stride samples of that noise: with 1000 samples (stride 1) instead
-        # of 10 the expected maximum of the rounding random walk is higher, and the kernel's working momenta
-        # pu = px + py, pv = px - py carry up to twice the ulp of px, py; the absolute part
-        # therefore grows as 2 sqrt(samples) ulp(E): +6 ulp at stride 100, +63 ulp at stride 1 (measured
-        # there: 65 ulp on the worst of 2211 trajectories, level 3 and level 0 alike).
-        xmax = math.pi + stride * abs(dt) * math.sqrt(2.0 * (cfg["E"] + 2.0 * cfg["eps"]))
-        tol = ((64 + 2 * math.sqrt(steps / stride)) * ULP1 * cfg["E"] * max(1.0, xmax / math.pi)
-               + 0.01 * st.acc[3, :n][live])
+        # dH_max: SURVEY 8(c)'s bar, 64 ulp(E) absolute + 1 % relative, unless an ORACLE-ONLY experiment on these
+        # very inputs shows that two correct implementations of the same map already differ by more than half of
+        # it: the oracle rebuilt with FMA contraction and every sin/cos moved by -1/0/+1 ulp (tests/jitter_trig.h;
+        # SURVEY App. B-6 style, no CUDA involved) gives the rounding noise N of dH_max for this scheme, step,
+        # stride and horizon; the absolute part of the bar is then max(64 ulp(E), 2 N).  Measured N:
+        # 7-9 ulp(E) for the order-4 cases at dt <= 0.007, 56 ulp(E) for (order 6, dt = 0.02, stride 1) where
+        # dH_max itself is 112 ulp(E) (pure rounding noise), 67 ulp(E) at dt = 0.05 where the angles reach 7 rad
+        # between wraps.
+        tol = max(64 * ULP1 * cfg["E"], 2.0 * noise) + 0.01 * st.acc[3, :n][live]
         dh = np.abs(got.acc[3, :n][live] - st.acc[3, :n][live])
         assert np.all(dh <= tol), (trig, (dh - tol).max())
 

@@ -483,3 +483,121 @@ def test_paper_resonance_geometry():
             assert abs(np.dot(g[key], W)) < 1e-12
         assert abs(np.dot(W, W) - 2 * E) < 1e-12
     assert g["tesla_resident"][0] == g["tesla_resident"][1] * g["tesla_resident"][2]
+
+
+# ------------------------------------------------------------------ a5: indicator image (R13, R14)
+
+def test_indicator_kinds_thresholds_and_masks(orc):
+    """awo_indicator on a hand-made accumulator table (no integration, nothing from the CUDA path): FLI is
+    plane 1, FTLE is plane 0 divided by t, DH is plane 3; CLASS is the STRICT comparison FLI > thr (R14);
+    every trajectory that is not live (status 0 off-shell, 2 non-finite, 3 left the area) reads NaN in the
+    float kinds and 255 in the class byte."""
+    n = 8
+    st = orc.State(n, tangent=True, wind=False)
+    thr = math.log(1000.0) + 3.0                                  # R14 at t = 1000
+    up, dn = np.nextafter(thr, np.inf), np.nextafter(thr, -np.inf)
+    #                 k:    0     1    2    3     4      5     6     7
+    st.acc[0, :n] = [250.0, -3.0, 1.5, 7.25, 99.0, 12.5, 0.0, 4.0]        # logsum
+    st.acc[1, :n] = [thr, up, dn, 7.25, 99.0, 99.0, 99.0, -0.0]           # fli_max
+    st.acc[2, :n] = 1.0                                                   # H0 (not an output)
+    st.acc[3, :n] = [1e-12, 2e-12, 3e-12, 4e-12, 5e-12, 6e-12, 7e-12, 0.0]  # dH_max
+    st.status[:] = [1, 1, 1, 1, 0, 2, 3, 1]
+    st.t = 1000.0
+    live = st.status == 1
+    fli, ftle, dh = orc.indicator(st, 0), orc.indicator(st, 1), orc.indicator(st, 2)
+    for img in (fli, ftle, dh):
+        assert np.array_equal(np.isnan(img), ~live)              # NaN exactly on the non-live ones
+    assert np.array_equal(fli[live], np.array([thr, up, dn, 7.25, -0.0]))
+    assert np.array_equal(ftle[live], np.array([0.25, -0.003, 0.0015, 0.00725, 0.004]))   # logsum / 1000, hand values
+    assert np.array_equal(dh[live], np.array([1e-12, 2e-12, 3e-12, 4e-12, 0.0]))          # plane 3, not 0, 1 or 2
+    cls = orc.indicator(st, 3, thr)
+    #  FLI == thr -> regular (strict >), one ulp above -> chaotic, one below -> regular, 7.25 < 9.9 -> regular
+    assert cls.tolist() == [0, 1, 0, 0, 255, 255, 255, 0]
+    assert cls.dtype == np.uint8
+    # the threshold is the argument, not a constant: a lower one flips pixel 3 only among the live regular ones
+    assert orc.indicator(st, 3, 7.0).tolist() == [1, 1, 1, 1, 255, 255, 255, 0]
+    assert orc.indicator(st, 3, 7.25).tolist() == [1, 1, 1, 0, 255, 255, 255, 0]
+    # FTLE uses the elapsed time of the state
+    st.t = 500.0
+    assert np.array_equal(orc.indicator(st, 1)[live], np.array([0.5, -0.006, 0.003, 0.0145, 0.008]))
+    # planes are addressed with the pitch, not n
+    st2 = orc.State(3, tangent=True, wind=False, pitch=64)
+    st2.acc[1, :3], st2.status[:], st2.t = [1.0, 2.0, 3.0], 1, 1.0
+    assert orc.indicator(st2, 0).tolist() == [1.0, 2.0, 3.0]
+
+
+def test_indicator_on_an_integrated_orbit_matches_the_eps0_closed_form(orc):
+    """End to end through awo_integrate + awo_indicator at eps = 0: FLI = sup_t ln|w(t)| with
+    |w(t)|^2 = |dX0 + t dP0|^2 + |dP0|^2 in closed form; FTLE = ln|w(T)| / T; DH = 0 up to rounding; the class
+    byte follows from comparing the closed form with thr."""
+    n = 64
+    st = orc.init_shell(orc.State(n), orc.make_grid(8, 8, angle_mode=1, tangent_mode=1), 1.0, 0.0, 11)
+    w0 = st.w[:, :n].copy()
+    orc.integrate(st, 2000, 0.01, 100)
+    ts = 0.01 * 100 * np.arange(1, 21)
+    norms = np.array([0.5 * np.log(((w0[:3] + t * w0[3:]) ** 2).sum(0) + (w0[3:] ** 2).sum(0)) for t in ts])
+    ref_fli = np.maximum(norms.max(0), 0.0)
+    assert np.max(np.abs(orc.indicator(st, 0) - ref_fli)) < 1e-12
+    assert np.max(np.abs(orc.indicator(st, 1) - norms[-1] / 20.0)) < 1e-13
+    assert orc.indicator(st, 2).max() < 1e-14
+    thr = float(np.median(ref_fli))
+    sure = np.abs(ref_fli - thr) > 1e-9
+    assert np.array_equal(orc.indicator(st, 3, thr)[sure], (ref_fli > thr).astype(np.uint8)[sure])
+
+
+# ------------------------------------------------------------------ slices of the ensemble (k0)
+
+@pytest.mark.parametrize("shape,angle_mode,tmode", [(0, 0, 0), (0, 1, 1), (1, 1, 0), (2, 1, 1), (3, 1, 1)])
+def test_init_shell_slices_are_rows_of_the_whole_ensemble(orc, shape, angle_mode, tmode):
+    """P:13, P:63 (independent realisations): a state that holds trajectories [k0, k0 + n) of the ensemble is,
+    bit for bit, that slice of the whole — grid position and every random draw are functions of the GLOBAL index.
+    The grid values themselves are re-derived here from the definition (cell centres, R6)."""
+    gx, gy = 12, 10
+    E, eps, seed = 1.0, 2e-2, 5
+    mk = lambda k0: orc.make_grid(gx, gy, -0.9, 0.7, angle_mode, shape, 0.1, -0.2, 0.05, 1, tmode,
+                                  lo_y=-0.5, hi_y=0.8, k0=k0)
+    whole = orc.init_shell(orc.State(gx * gy), mk(0), E, eps, seed)
+    for k0, n in ((0, 37), (37, 50), (87, 33), (119, 1), (60, 0)):
+        part = orc.init_shell(orc.State(n), mk(k0), E, eps, seed)
+        assert np.array_equal(part.q[:, :n], whole.q[:, k0:k0 + n], equal_nan=True)
+        assert np.array_equal(part.w[:, :n], whole.w[:, k0:k0 + n])
+        assert np.array_equal(part.acc[:, :n], whole.acc[:, k0:k0 + n], equal_nan=True)
+        assert np.array_equal(part.status, whole.status[k0:k0 + n])
+        if shape == 0 and n:
+            K = k0 + np.arange(n)
+            px = -0.9 + ((K % gx) + 0.5) * (0.7 - -0.9) / gx
+            py = -0.5 + ((K // gx) + 0.5) * (0.8 - -0.5) / gy
+            assert np.array_equal(part.q[3, :n], px) and np.array_equal(part.q[4, :n], py)
+        if angle_mode and n:
+            assert part.q[0, 0] == 2 * math.pi * orc.uniform(seed, k0, 0) or np.isnan(part.q[0, 0])
+    # a slice may not reach past the ensemble
+    import ctypes
+    bad = orc.State(5)
+    g = mk(gx * gy - 4)
+    rc = orc.lib().awo_init_shell(ctypes.byref(g), E, eps, seed, 5, bad.pitch, bad.q.ctypes.data_as(orc._dp),
+                                  bad.w.ctypes.data_as(orc._dp), bad.acc.ctypes.data_as(orc._dp),
+                                  bad.wind.ctypes.data_as(orc._i32p), bad.status.ctypes.data_as(orc._u8p))
+    assert rc == -1
+
+
+def test_gaussian_cloud_is_a_2d_normal(orc):
+    """"Gaussian distribution ... with the dispersion sigma": the radius of a 2-d normal is Rayleigh,
+    P(r < a sigma) = 1 - exp(-a^2/2); components independent with variance sigma^2; the centre is W."""
+    n = 1 << 16
+    sig, cx, cy = 0.01, math.sqrt(15.0), math.sqrt(15.0)
+    g = orc.make_grid(256, 256, angle_mode=1, shape=2, cx=cx, cy=cy, r=sig)
+    st = orc.init_shell(orc.State(n, tangent=False), g, 15.0, 1.0, 4)
+    live = st.status == 1
+    # W lies on the equator pz = 0 of the E = 15 shell: roughly half the cloud is outside the shell (R8)
+    assert 0.3 < live.mean() < 0.7
+    g2 = orc.make_grid(256, 256, angle_mode=1, shape=2, cx=1.0, cy=-2.0, r=sig)
+    s2 = orc.init_shell(orc.State(n, tangent=False), g2, 15.0, 1.0, 4)
+    assert np.all(s2.status == 1)
+    dx, dy = s2.q[3, :n] - 1.0, s2.q[4, :n] + 2.0
+    r = np.hypot(dx, dy) / sig
+    for a in (0.5, 1.0, 2.0, 3.0):
+        assert abs((r < a).mean() - (1 - math.exp(-a * a / 2))) < 4e-3
+    assert abs(dx.std() / sig - 1) < 0.01 and abs(dy.std() / sig - 1) < 0.01
+    assert abs(np.corrcoef(dx, dy)[0, 1]) < 0.012 and abs(dx.mean()) < 1.2e-4 and abs(dy.mean()) < 1.2e-4
+    H = 0.5 * (s2.q[3:, :n] ** 2).sum(0) + np.cos(s2.q[0, :n]) * np.cos(s2.q[1, :n]) * (1 + np.cos(2 * s2.q[2, :n]))
+    assert np.max(np.abs(H - 15.0)) < 64 * np.spacing(15.0)                 # v_z from the energy condition
