@@ -18,7 +18,7 @@
  *   - returns an aw_status (0 = AW_OK, negative = error); never throws, never sets errno;
  *   - every argument is validated ON THE HOST before anything is launched;
  *   - all device work is enqueued asynchronously on aw_state.stream; no call synchronises unless its
- *     comment says so (the *_host and *_probe calls do);
+ *     comment says so (aw_bound_energy and the *_host calls do);
  *   - the library never allocates or frees the caller's planes; pointers marked "device" must be
  *     device-accessible global memory, 16-byte aligned; "host" pointers are ordinary host memory;
  *   - thread-safe for distinct aw_state objects; the only library state is a thread-local
@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define AW_VERSION 120 /* 1.2.0 */
+#define AW_VERSION 200 /* 2.0.0: aw_grid.k0, aw_state.Emax / block, AW_ST_RANGE, aw_bound_energy; probes moved out */
 
 #if defined(__GNUC__)
 #define AW_API __attribute__((visibility("default")))
@@ -59,7 +59,8 @@ enum { AW_DENS_ACTION = 0, AW_DENS_VEL_UPPER = 1, AW_DENS_VEL_LOWER = 2, AW_DENS
 /* aw_grid.shape */
 enum { AW_SHAPE_GRID = 0, AW_SHAPE_DISK = 1, AW_SHAPE_GAUSS = 2, AW_SHAPE_SPHERE = 3 };
 /* per-trajectory status byte */
-enum { AW_ST_OFFSHELL = 0, AW_ST_LIVE = 1, AW_ST_NONFINITE = 2, AW_ST_LEFT = 3 };
+enum { AW_ST_OFFSHELL = 0, AW_ST_LIVE = 1, AW_ST_NONFINITE = 2, AW_ST_LEFT = 3,
+       AW_ST_RANGE = 4 /* energy above the bound aw_integrate was launched for (see aw_state.Emax): not integrated */ };
 
 /* Static, never-freed description of a status code. */
 AW_API const char *aw_strerror(int code);
@@ -97,11 +98,20 @@ typedef struct {
   double surv_lo_x, surv_hi_x, surv_lo_y, surv_hi_y; /* launch rectangle of the survivor filter:
                       a trajectory whose (px, py) is outside [lo_x, hi_x) x [lo_y, hi_y) at a
                       checkpoint gets status AW_ST_LEFT and is frozen there                    */
+  double Emax;     /* upper bound of H(X,P) over the live trajectories (P^2 <= 2(H + 2|eps|) on the whole orbit).
+                      aw_integrate sizes its arithmetic (trigonometry level, angle range) for max(E, Emax) and CHECKS
+                      it on the device: a trajectory with H above what the launch supports gets AW_ST_RANGE and is left
+                      untouched, never integrated inaccurately.  aw_init_shell sets it to E; aw_bound_energy sets it
+                      from the data (uploaded states); 0 / NaN = use E                              */
+  int32_t block;   /* threads per block of the integrator: 0 (default) = chosen from n so that small ensembles
+                      spread over all SMs; 32, 64 or 128 = forced.  The result does not depend on it    */
+  int32_t reserved_;
 } aw_state;
 
 /* Initial-condition family (P:85 whole region, P:87 patch, P:97 cloud; R6, R8, R9, R12, R17, R18). */
 typedef struct {
-  int32_t gx, gy;               /* n must equal gx*gy; trajectory k = j*gx + i                 */
+  int32_t gx, gy;               /* the WHOLE ensemble: gx*gy trajectories, trajectory K = j*gx + i; the state
+                                   holds the slice K in [k0, k0 + n), element k = K - k0 of its planes    */
   double lo_x, hi_x, lo_y, hi_y; /* action rectangle for shape GRID; samples are cell-centred:
                                     px = lo_x + (i + 1/2)(hi_x - lo_x)/gx, py likewise with j  */
   int32_t angle_mode;           /* 0: all angles 0;  1: angle_a = 2pi * u(seed, k, a), a=0,1,2 */
@@ -114,6 +124,10 @@ typedef struct {
   double cx, cy, r;
   int32_t pz_sign;              /* +1 (default, upper hemisphere; R9) or -1                    */
   int32_t tangent_mode;         /* 0: one common seeded unit vector (R12); 1: per trajectory   */
+  int64_t k0;                   /* first trajectory of the slice this state holds (0 for the whole ensemble).  Grid
+                                   position and every random draw are functions of the GLOBAL index K, so a slice
+                                   is bit-identical to the same rows of the whole (multi-GPU sharding, P:13, P:63;
+                                   R30): rank r of a row-sharded job passes k0 = j0*gx, n = rows*gx          */
 } aw_grid;
 
 /* Bytes the caller must provide for each buffer.  *pitch_out = n rounded up to a multiple of 32.
@@ -123,15 +137,15 @@ AW_API size_t aw_state_bytes(int64_t n, int with_tangent, int with_wind, int64_t
 
 /* Counter-based randomness (R11): mix64(seed, ctr): z = seed + ctr*0x9E3779B97F4A7C15 (mod 2^64);
  * z ^= z>>30; z *= 0xBF58476D1CE4E5B9; z ^= z>>27; z *= 0x94D049BB133111EB; z ^= z>>31.
- * u(seed, k, slot) = (mix64(seed, 16k + slot) >> 11) * 2^-53 in [0,1).  Slots: 0-2 angles, 3-4 cloud,
+ * u(seed, K, slot) = (mix64(seed, 16K + slot) >> 11) * 2^-53 in [0,1), K the global index.  Slots: 0-2 angles, 3-4 cloud,
  * 5-10 tangent normals (Box-Muller pairs (5,6), (7,8), (9,10) on (1 - u_a, u_b)).                 */
 
 /* §8(a) a1 — initial conditions on the energy shell ("v_z from the energy
- * condition").  For every k: (px,py) from the grid or cloud; angles per angle_mode;
+ * condition").  For every K = k0 + k, k in [0, n): (px,py) from the grid or cloud; angles per angle_mode;
  * R = 2(E - eps H_p(X)) - px^2 - py^2; R < 0 -> status 0 and all six state words NaN (R8);
  * else pz = pz_sign*sqrt(R), status 1.  acc = {0, 0, H(X,P), 0}; wind = 0; tangent = common unit
  * vector (computed on the host, see aw_common_tangent) or the per-trajectory one.  Sets s->E, eps,
- * t = 0, step = 0, ready = 1.  Errors: AW_EINVAL (null s/grid/planes, n != gx*gy, pitch < n or not a
+ * Emax = E, t = 0, step = 0, ready = 1.  Errors: AW_EINVAL (null s/grid/planes, k0 < 0 or k0 + n > gx*gy, pitch < n or not a
  * multiple of 32, hi <= lo, r < 0, bad modes), AW_ERANGE (E - 2|eps| <= 0 or non-finite). */
 AW_API int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps, uint64_t seed);
 
@@ -154,7 +168,11 @@ AW_API int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps,
  * with the drift angle d = a_s p (Taylor polynomials in d; the degree is picked on the host from
  * max_s |a_s| sqrt(2(E + 2|eps|)) so the truncation stays below 2^-60; aw_trig_level reports it), and
  * recomputes them from the angles with the device sincos at every checkpoint and at least every 128
- * steps.  s->E must therefore bound the energy of an uploaded state.  If the drift angle can exceed
+ * steps.  The bound is max(s->E, s->Emax) and it is ENFORCED: every call first runs one elementwise kernel that
+ * evaluates each live trajectory's H(X,P) and compares it with the largest energy the chosen level (and the angle
+ * range of R7) supports; above it the trajectory gets AW_ST_RANGE and is not touched (P^2 <= 2(H + 2|eps|)
+ * along the whole orbit, so the check before the first step covers every step).  Call aw_bound_energy after uploading a state whose
+ * energy the struct does not know.  If the drift angle can exceed
  * 0.357 rad the kernel is mixed (levels 8 and 9, up to 0.54 and 2 rad): the scheme's shorter drifts still rotate the
  * pairs, the long ones are followed by the device sincos; beyond 2 rad, or with s->trig == 1, the device sincos is evaluated at
  * every stage (level 0).
@@ -177,7 +195,7 @@ AW_API int aw_mark(aw_state *s);
  * §8(f): AW_IND_DP: |P - Pref| (three rounded squares summed left to right, IEEE sqrt).
  * AW_IND_VX / VY / VZ: component of the projected averaged velocity Vhat (see aw_density), NaN where
  * the trajectory is not live or |V| = 0.  These need s->qref (AW_ESTATE if NULL); VX..VZ also need
- * s->t > s->tref.
+ * s->wind, s->windref and s->t > s->tref.
  * AW_IND_DHS: the signed energy error of the CURRENT state, H(X,P) - H0, by the routine the checkpoint uses
  * (BASELINE configs[2] "energy-drift statistics"; R29). */
 AW_API int aw_indicator(const aw_state *s, int kind, double thr, void *out_dev);
@@ -193,8 +211,8 @@ AW_API int aw_energy_stats(const aw_state *s, void *scratch_dev, double *out_dev
 
 /* §8(a) a6 — visited-cell density over the first two actions (R19, R20).  For each live
  * trajectory ix = floor((px - lo) * (gx/(hi - lo))), iy likewise with gy; inside -> hist[iy*gx + ix]
- * += 1, else *dropped_dev += 1 (dropped_dev may be NULL).  ADDS into hist_dev (device, gx*gy uint32;
- * the caller zeroes it) so repeated calls give the time-accumulated density.
+ * += 1, else *dropped_dev += 1 (dropped_dev may be NULL; 8-byte aligned).  ADDS into hist_dev (device, gx*gy
+ * uint32, 4-byte aligned; the caller zeroes it) so repeated calls give the time-accumulated density.
  * mode AW_DENS_ACTION (0): the point binned is the instantaneous (px, py) (BASELINE configs[4]).
  * modes 1-3, §8(f) 1 — the paper's own indicator (P:67, P:171 fn. 26; R26, R27): the point binned is
  * (Vhat_x, Vhat_y) of the averaged finite-time velocity over the window [tref, t] since aw_mark,
@@ -203,9 +221,17 @@ AW_API int aw_energy_stats(const aw_state *s, void *scratch_dev, double *out_dev
  * every operation rounded separately in this order (no FMA), i.e. the sphere S seen along the third
  * axis: AW_DENS_VEL_UPPER counts the hemisphere Vhat_z >= 0, _LOWER Vhat_z < 0, _BOTH both (folded);
  * the other hemisphere, |V| = 0 or non-finite, and points outside [lo, hi)^2 go to *dropped_dev.
- * AW_ESTATE if s->qref == NULL or !(s->t > s->tref). */
+ * AW_ESTATE if s->qref, s->wind or s->windref is NULL (without turn counters a trajectory that completed a turn
+ * inside the window would alias silently) or !(s->t > s->tref).  AW_EINVAL for misaligned hist_dev / dropped_dev. */
 AW_API int aw_density(const aw_state *s, uint32_t *hist_dev, int32_t gx, int32_t gy, double lo, double hi,
                int mode, uint64_t *dropped_dev);
+
+/* Largest energy among the live trajectories, from the data (SYNCHRONOUS: one reduction kernel, an 8-byte copy
+ * and a stream synchronise): s->Emax <- max over live k of H(X_k, P_k) by the routine the checkpoint uses.  For
+ * states the library did not initialise (uploaded planes, aw_map_host): afterwards aw_integrate picks the
+ * trigonometry level from the data instead of trusting s->E.  scratch_dev: 8 bytes of device memory, 8-byte
+ * aligned.  An ensemble without live trajectories leaves Emax unchanged.  Needs s->eps set and ready. */
+AW_API int aw_bound_energy(aw_state *s, void *scratch_dev);
 
 /* Host helpers (pure host arithmetic, no device needed) ------------------------------------------ */
 
@@ -218,6 +244,10 @@ AW_API int aw_stage_constants(int order, double dt, double eps, double *a_host, 
  * (6,7), (7,8), 8 and 9 = mixed (rotations through the shorter drifts, device sincos after the long ones); or a
  * negative aw_status.  Pure host arithmetic. */
 AW_API int aw_trig_level(const aw_state *s, double dt);
+/* Threads per block aw_integrate launches for this state: s->block if forced, else 128 when ceil(n/128) fills every
+ * SM with its 4 resident blocks, else 64 or 32 so that a small ensemble's warps spread over all SMs (queries the
+ * current device's SM count; 148 if there is none).  The result of aw_integrate does not depend on it. */
+AW_API int aw_block_size(const aw_state *s);
 /* The common tangent vector of tangent_mode 0: unit vector from u(seed, 2^63-1, 5..10) (R12). */
 AW_API int aw_common_tangent(uint64_t seed, double *t6_host);
 
@@ -228,7 +258,12 @@ AW_API int aw_common_tangent(uint64_t seed, double *t6_host);
  * (n doubles, or n bytes for CLASS) and the histogram (gx*gy uint32, ADDED into hist_host's content
  * is NOT done: the device histogram is zeroed first and hist_host is overwritten) and the final state
  * planes that are non-NULL in the out arguments.  ind_dev / hist_dev are device scratch of n*8 and
- * gx*gy*4 + 8 bytes.  Synchronises s->stream before returning. */
+ * AW_HIST_SCRATCH_BYTES(gx, gy) = gx*gy*4 rounded up to a multiple of 8, + 8 bytes (histogram, then the 64-bit
+ * dropped counter, 8-byte aligned whatever the parity of gx*gy).  Every argument is validated before the first
+ * copy is enqueued; the trigonometry level is picked from the uploaded data (aw_bound_energy); on any failure
+ * after work was enqueued the stream is synchronised before returning, so the host buffers are always free
+ * again when the call returns.  Synchronises s->stream before returning. */
+#define AW_HIST_SCRATCH_BYTES(gx, gy) ((((size_t)(gx) * (size_t)(gy) * 4 + 7) / 8) * 8 + 8)
 typedef struct {
   const double *q, *w, *acc;  /* host, same pitch as s                                            */
   const int32_t *wind;        /* host or NULL                                                     */
@@ -250,34 +285,10 @@ AW_API int aw_map_host(aw_state *s, const aw_host_in *in, int64_t steps, double 
  * aw_map_host does, takes the snapshot (aw_mark: the state is the X(t) of the window), runs aw_integrate(steps, dt,
  * stride) — the averaging window Dt = steps*|dt| — then aw_density(mode 1..3) of the projected averaged velocity into
  * the zeroed device histogram, and downloads it (gx*gy uint32) plus out->dropped / q / acc / status where non-NULL;
- * out->image is ignored.  hist_dev: device scratch of gx*gy*4 + 8 bytes.  s must carry qref (and windref iff wind). */
+ * out->image is ignored.  hist_dev: device scratch of AW_HIST_SCRATCH_BYTES(gx, gy).  s must carry qref, wind and windref. */
 AW_API int aw_velocity_map_host(aw_state *s, const aw_host_in *in, int64_t steps, double dt, int64_t stride, int mode,
                                 int32_t gx, int32_t gy, double lo, double hi, void *hist_dev,
                                 const aw_host_out *out);
-
-/* Probes (synchronous; test and measurement support, not on the hot path) ------------------------ */
-
-/* Device sincos used by the integrator (csrc/aw_trig.cuh), evaluated on n device doubles. */
-AW_API int aw_sincos_probe(const double *x_dev, int64_t n, double *sin_dev, double *cos_dev, void *stream);
-/* u(seed, k0 + i, slot) for i in [0, n) written to out_dev (device). */
-AW_API int aw_uniform_probe(uint64_t seed, uint64_t k0, int64_t n, uint32_t slot, double *out_dev,
-                     void *stream);
-/* H(X,P) by the device routine the checkpoint uses, for n states in SoA planes q (6*pitch). */
-AW_API int aw_hamiltonian_probe(const double *q_dev, int64_t n, int64_t pitch, double eps, double *out_dev,
-                         void *stream);
-/* fp64 FMA peak microbenchmark: every thread runs `chains` (1..16) independent DFMA chains of `iters`
- * links; grid = blocks x threads.  Writes elapsed milliseconds (CUDA events) and the DFMA count
- * (thread-instructions) to the host outputs; flop/s = 2*dfma/ms*1e3.  sink_dev: >= 8 bytes device. */
-AW_API int aw_dfma_peak_probe(int blocks, int threads, int chains, int64_t iters, double *sink_dev,
-                       double *ms_host, double *dfma_host, void *stream);
-
-/* fp64 issue rate by operand shape (the register-operand bandwidth behind DESIGN.md §6.1): every thread
- * runs 8 independent chains, 32 fp64 instructions per loop trip, `iters` trips.  shape 0: fma(v, u0, w0),
- * two register operands shared by neighbouring instructions; 1: fma(v, u_c, w_c), three distinct registers;
- * 2: fma(v, u_c, immediate); 3: fma(v, v, w_c); 4: v * u_c (DMUL); 5: fma(u_c, w_c', v).  Writes elapsed
- * milliseconds and the fp64 thread-instruction count to the host outputs.  work_dev: >= 136 doubles. */
-AW_API int aw_dfma_shape_probe(int blocks, int threads, int shape, int64_t iters, double *work_dev,
-                               double *ms_host, double *inst_host, void *stream);
 
 #ifdef __cplusplus
 }

@@ -17,7 +17,7 @@ AW_IND_FLI, AW_IND_FTLE, AW_IND_DH, AW_IND_CLASS = 0, 1, 2, 3
 AW_IND_DP, AW_IND_VX, AW_IND_VY, AW_IND_VZ, AW_IND_DHS = 4, 5, 6, 7, 8
 AW_DENS_ACTION, AW_DENS_VEL_UPPER, AW_DENS_VEL_LOWER, AW_DENS_VEL_BOTH = 0, 1, 2, 3
 AW_SHAPE_GRID, AW_SHAPE_DISK, AW_SHAPE_GAUSS, AW_SHAPE_SPHERE = 0, 1, 2, 3
-AW_ST_OFFSHELL, AW_ST_LIVE, AW_ST_NONFINITE, AW_ST_LEFT = 0, 1, 2, 3
+AW_ST_OFFSHELL, AW_ST_LIVE, AW_ST_NONFINITE, AW_ST_LEFT, AW_ST_RANGE = 0, 1, 2, 3, 4
 
 
 class AwError(RuntimeError):
@@ -38,7 +38,8 @@ class AwState(C.Structure):
                 ("stream", C.c_void_p),
                 ("qref", C.c_void_p), ("windref", C.c_void_p), ("tref", C.c_double),
                 ("surv_lo_x", C.c_double), ("surv_hi_x", C.c_double),
-                ("surv_lo_y", C.c_double), ("surv_hi_y", C.c_double)]
+                ("surv_lo_y", C.c_double), ("surv_hi_y", C.c_double),
+                ("Emax", C.c_double), ("block", C.c_int32), ("reserved_", C.c_int32)]
 
 
 class Grid(C.Structure):
@@ -46,7 +47,7 @@ class Grid(C.Structure):
                 ("lo_x", C.c_double), ("hi_x", C.c_double), ("lo_y", C.c_double), ("hi_y", C.c_double),
                 ("angle_mode", C.c_int32), ("shape", C.c_int32),
                 ("cx", C.c_double), ("cy", C.c_double), ("r", C.c_double),
-                ("pz_sign", C.c_int32), ("tangent_mode", C.c_int32)]
+                ("pz_sign", C.c_int32), ("tangent_mode", C.c_int32), ("k0", C.c_int64)]
 
 
 class HostIn(C.Structure):
@@ -60,9 +61,11 @@ class HostOut(C.Structure):
 
 
 def make_grid(gx, gy, lo=-1.0, hi=1.0, angle_mode=0, shape=0, cx=0.0, cy=0.0, r=0.0, pz_sign=1,
-              tangent_mode=0, lo_y=None, hi_y=None):
+              tangent_mode=0, lo_y=None, hi_y=None, k0=0):
+    """The grid describes the WHOLE ensemble of gx*gy trajectories; an Ensemble of n trajectories initialised with
+    it holds the slice [k0, k0 + n) (include/aw.h, aw_grid.k0)."""
     return Grid(gx, gy, lo, hi, lo if lo_y is None else lo_y, hi if hi_y is None else hi_y,
-                angle_mode, shape, cx, cy, r, pz_sign, tangent_mode)
+                angle_mode, shape, cx, cy, r, pz_sign, tangent_mode, k0)
 
 
 _lib = None
@@ -99,12 +102,8 @@ def lib():
                                   i32, i32, dbl, dbl, vp, vp, C.POINTER(HostOut)]
         L.aw_velocity_map_host.argtypes = [C.POINTER(AwState), C.POINTER(HostIn), i64, dbl, i64, C.c_int, i32, i32,
                                            dbl, dbl, vp, C.POINTER(HostOut)]
-        L.aw_sincos_probe.argtypes = [vp, i64, vp, vp, vp]
-        L.aw_uniform_probe.argtypes = [u64, u64, i64, C.c_uint32, vp, vp]
-        L.aw_hamiltonian_probe.argtypes = [vp, i64, i64, dbl, vp, vp]
-        L.aw_dfma_peak_probe.argtypes = [C.c_int, C.c_int, C.c_int, i64, vp, C.POINTER(dbl),
-                                         C.POINTER(dbl), vp]
-        L.aw_dfma_shape_probe.argtypes = [C.c_int, C.c_int, C.c_int, i64, vp, C.POINTER(dbl), C.POINTER(dbl), vp]
+        L.aw_bound_energy.argtypes = [C.POINTER(AwState), vp]
+        L.aw_block_size.argtypes = [C.POINTER(AwState)]
         _lib = L
     return _lib
 
@@ -155,6 +154,10 @@ def aw_trig_level(ens, dt):
     return _check(lib().aw_trig_level(C.byref(ens.c), dt), "aw_trig_level")
 
 
+def aw_block_size(ens):
+    return _check(lib().aw_block_size(C.byref(ens.c)), "aw_block_size")
+
+
 def aw_common_tangent(seed):
     t = (C.c_double * 6)()
     _check(lib().aw_common_tangent(seed, t), "aw_common_tangent")
@@ -192,6 +195,7 @@ class Ensemble:
     t = property(lambda s: s.c.t)
     step = property(lambda s: s.c.step)
     tref = property(lambda s: s.c.tref)
+    Emax = property(lambda s: s.c.Emax)
 
     def set_survivors(self, rect):
         """rect = (lo_x, hi_x, lo_y, hi_y) switches the survivor filter of P:99 on; None switches it off."""
@@ -208,6 +212,14 @@ class Ensemble:
     @order.setter
     def order(self, v):
         self.c.order = v
+
+    @property
+    def block(self):
+        return self.c.block
+
+    @block.setter
+    def block(self, v):
+        self.c.block = v
 
     @property
     def trig(self):
@@ -229,7 +241,7 @@ class Ensemble:
         if self.wind is not None and wind is not None:
             self.wind.copy_(torch.from_numpy(wind))
         self.status[:self.n].copy_(torch.from_numpy(status))
-        self.c.E, self.c.eps, self.c.t, self.c.step, self.c.ready = E, eps, t, step, 1
+        self.c.E, self.c.Emax, self.c.eps, self.c.t, self.c.step, self.c.ready = E, E, eps, t, step, 1
 
 
 def aw_init_shell(ens, grid, E, eps, seed, stream=None):
@@ -242,6 +254,14 @@ def aw_integrate(ens, n, steps, dt, stride, stream=None):
     ens.bind_stream(stream)
     _check(lib().aw_integrate(C.byref(ens.c), n, steps, dt, stride), "aw_integrate")
     return ens
+
+
+def aw_bound_energy(ens, stream=None):
+    """Synchronous: ens.Emax <- max over live trajectories of H(X,P), from the data (include/aw.h)."""
+    ens.bind_stream(stream)
+    scratch = torch.zeros((1,), dtype=torch.int64, device=ens.device)
+    _check(lib().aw_bound_energy(C.byref(ens.c), _ptr(scratch)), "aw_bound_energy")
+    return ens.c.Emax
 
 
 def aw_mark(ens, stream=None):
@@ -306,42 +326,3 @@ def aw_velocity_map_host(ens, host_in, steps, dt, stride, mode, hist_shape, lo, 
     gy, gx = hist_shape
     _check(lib().aw_velocity_map_host(C.byref(ens.c), C.byref(hin), steps, dt, stride, mode, gx, gy, lo, hi,
                                       _ptr(hist_dev), C.byref(hout)), "aw_velocity_map_host")
-
-
-# ------------------------------------------------------------------------------ probes
-
-def aw_sincos_probe(x):
-    s, c = torch.empty_like(x), torch.empty_like(x)
-    _check(lib().aw_sincos_probe(_ptr(x), x.numel(), _ptr(s), _ptr(c), _stream_ptr()), "aw_sincos_probe")
-    return s, c
-
-
-def aw_uniform_probe(seed, k0, n, slot, device="cuda:0"):
-    out = torch.empty((n,), dtype=torch.float64, device=device)
-    _check(lib().aw_uniform_probe(seed, k0, n, slot, _ptr(out), _stream_ptr()), "aw_uniform_probe")
-    return out
-
-
-def aw_hamiltonian_probe(q, n, pitch, eps):
-    out = torch.empty((n,), dtype=torch.float64, device=q.device)
-    _check(lib().aw_hamiltonian_probe(_ptr(q), n, pitch, eps, _ptr(out), _stream_ptr()),
-           "aw_hamiltonian_probe")
-    return out
-
-
-def aw_dfma_peak_probe(blocks, threads, chains, iters, device="cuda:0"):
-    """Returns (milliseconds, DFMA thread-instructions)."""
-    sink = torch.zeros((2,), dtype=torch.float64, device=device)
-    ms, cnt = C.c_double(0), C.c_double(0)
-    _check(lib().aw_dfma_peak_probe(blocks, threads, chains, iters, _ptr(sink), C.byref(ms),
-                                    C.byref(cnt), _stream_ptr()), "aw_dfma_peak_probe")
-    return ms.value, cnt.value
-
-
-def aw_dfma_shape_probe(blocks, threads, shape, iters, device="cuda:0"):
-    """Returns (milliseconds, fp64 thread-instructions) for one operand shape (include/aw.h)."""
-    work = torch.zeros((160,), dtype=torch.float64, device=device)
-    ms, cnt = C.c_double(0), C.c_double(0)
-    _check(lib().aw_dfma_shape_probe(blocks, threads, shape, iters, _ptr(work), C.byref(ms), C.byref(cnt),
-                                     _stream_ptr()), "aw_dfma_shape_probe")
-    return ms.value, cnt.value

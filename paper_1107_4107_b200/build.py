@@ -29,6 +29,18 @@ def _nvcc():
     raise RuntimeError("nvcc not found")
 
 
+def source_hash():
+    """16 hex digits identifying what libaw.so is built from: every source, header and the compiler flags.  bench.py
+    quotes an ncu-measured DRAM traffic figure only when it was captured on the same build (profiles/traffic_by_build.csv)."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(set(SOURCES + HEADERS)):
+        h.update(f.encode())
+        h.update(open(os.path.join(CSRC, f), "rb").read())
+    h.update(repr((NVCC_FLAGS, UNITS)).encode())
+    return h.hexdigest()[:16]
+
+
 def needs_build():
     if not os.path.exists(LIB):
         return True

@@ -174,6 +174,14 @@ static int check_planes(const aw_state *s) {
 
 // the marked snapshot is usable: planes present, wind/windref paired
 static bool has_ref(const aw_state *s) { return s->qref && ((s->wind == nullptr) == (s->windref == nullptr)); }
+// the averaged velocity needs the turn counters too: without them a trajectory that completed a turn inside the
+// window would alias silently (the checkpoint wraps the angles whether or not the turns are counted)
+static bool has_velocity_ref(const aw_state *s) { return s->qref && s->wind && s->windref; }
+
+static bool aligned(const void *p, uintptr_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
+
+// energy bound the arithmetic is sized for: max(E, Emax); Emax = 0 / NaN / smaller means "use E"
+static double energy_bound(const aw_state *s) { return (s->Emax > s->E) ? s->Emax : s->E; }
 
 static VelocityArgs velocity_args(const aw_state *s) {
   VelocityArgs v;
@@ -233,7 +241,13 @@ int aw_trig_level(const aw_state *s, double dt) {
   const int S = stage_constants(s->order, dt, s->eps, a, b);
   double amax = std::fmax(std::fabs(a[0]), std::fmax(std::fabs(a[S]), std::fabs(a[S] + a[0])));
   for (int k = 1; k < S; ++k) amax = std::fmax(amax, std::fabs(a[k]));
-  return trig_level_for(amax * std::sqrt(2.0 * (s->E + 2.0 * std::fabs(s->eps))));
+  return trig_level_for(amax * std::sqrt(2.0 * (energy_bound(s) + 2.0 * std::fabs(s->eps))));
+}
+
+int aw_block_size(const aw_state *s) {
+  if (!s || s->n < 0) return AW_EINVAL;
+  if (s->block != 0 && s->block != 32 && s->block != 64 && s->block != 128) return AW_EINVAL;
+  return integrate_block_size(s->n, s->block);
 }
 
 int aw_common_tangent(uint64_t seed, double *t6_host) {
@@ -246,7 +260,8 @@ int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps, uint64
   if (!s || !grid) return AW_EINVAL;
   int rc = check_planes(s);
   if (rc != AW_OK) return rc;
-  if (grid->gx <= 0 || grid->gy <= 0 || (int64_t)grid->gx * grid->gy != s->n) return AW_EINVAL;
+  if (grid->gx <= 0 || grid->gy <= 0) return AW_EINVAL;
+  if (grid->k0 < 0 || grid->k0 > (int64_t)grid->gx * grid->gy - s->n) return AW_EINVAL;  // slice inside the ensemble
   if (grid->angle_mode != 0 && grid->angle_mode != 1) return AW_EINVAL;
   if (grid->tangent_mode != 0 && grid->tangent_mode != 1) return AW_EINVAL;
   if (grid->shape == AW_SHAPE_GRID) {
@@ -271,7 +286,7 @@ int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps, uint64
     common_tangent(seed, p.tcommon);
     AW_CUDA(launch_init(p, (cudaStream_t)s->stream));
   }
-  s->E = E; s->eps = eps; s->t = 0.0; s->step = 0; s->ready = 1;
+  s->E = E; s->Emax = E; s->eps = eps; s->t = 0.0; s->step = 0; s->ready = 1;
   if (s->order != 4 && s->order != 6) s->order = 4;
   return AW_OK;
 }
@@ -285,7 +300,8 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
   if (!s->ready || (s->order != 4 && s->order != 6)) return AW_ESTATE;
   if (!std::isfinite(s->E) || !std::isfinite(s->eps)) return AW_ESTATE;
   if (stride > 0x7fffffff) return AW_ERANGE;
-  const double vmax = std::sqrt(2.0 * (s->E + 2.0 * std::fabs(s->eps)));
+  if (s->block != 0 && s->block != 32 && s->block != 64 && s->block != 128) return AW_EINVAL;
+  const double vmax = std::sqrt(2.0 * (energy_bound(s) + 2.0 * std::fabs(s->eps)));
   if (!((double)stride * std::fabs(dt) * vmax < 1024.0)) return AW_ERANGE;
   if (steps == 0 || n == 0) return AW_OK;
 
@@ -316,6 +332,17 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
   for (int k = 0; k < S; ++k) amax = std::fmax(amax, std::fabs(p.a_loop[k]));
   p.level = s->trig ? 0 : trig_level_for(amax * vmax);
   if (p.level > 0 && (amax != std::fabs(p.a_loop[S - 1]) || !drift_ratios_hold(S, p.a_loop))) p.level = 0;
+  // the largest |P| this launch's arithmetic supports: the Taylor degrees of the level (kLevelMaxD / amax) and the
+  // exact range of the two-constant argument reduction (R7: stride |dt| |P| < 1024); as an energy, P^2 <= 2(H + 2|eps|)
+  {
+    const double v_level = trig_level_max_angle(p.level) / amax;
+    const double v_range = 1024.0 / ((double)stride * std::fabs(dt));
+    const double v = std::fmin(v_level, v_range);
+    const double hmax = 0.5 * v * v - 2.0 * std::fabs(s->eps);
+    const cudaError_t e = launch_range_check(s->q, s->status, s->n, s->pitch, s->eps, hmax, (cudaStream_t)s->stream);
+    if (e != cudaSuccess) return cuda_fail(e);
+  }
+  p.block = integrate_block_size(s->n, s->block);
   const int64_t pieces = (stride + kMaxChunk - 1) / kMaxChunk;
   p.chunk = (int32_t)((stride + pieces - 1) / pieces);
 
@@ -366,7 +393,7 @@ int aw_indicator(const aw_state *s, int kind, double thr, void *out_dev) {
   }
   if (kind >= AW_IND_DP) {
     if (!has_ref(s)) return AW_ESTATE;
-    if (kind != AW_IND_DP && !(s->t > s->tref)) return AW_ESTATE;
+    if (kind != AW_IND_DP && (!has_velocity_ref(s) || !(s->t > s->tref))) return AW_ESTATE;
     if (!aligned16(out_dev)) return AW_EINVAL;
     if (s->n == 0) return AW_OK;
     AW_CUDA(launch_indicator_ref(velocity_args(s), s->status, s->n, kind, static_cast<double *>(out_dev),
@@ -410,13 +437,92 @@ int aw_density(const aw_state *s, uint32_t *hist_dev, int32_t gx, int32_t gy, do
     return AW_EINVAL;
   if ((int64_t)gx * gy >= 0xffffffffll) return AW_ERANGE;
   if (!s->ready) return AW_ESTATE;
-  if (mode != AW_DENS_ACTION && (!has_ref(s) || !(s->t > s->tref))) return AW_ESTATE;
+  if (!aligned(hist_dev, 4) || !aligned(dropped_dev, 8)) return AW_EINVAL;
+  if (mode != AW_DENS_ACTION && (!has_velocity_ref(s) || !(s->t > s->tref))) return AW_ESTATE;
   if (s->n == 0) return AW_OK;
   const double fx = (double)gx / (hi - lo), fy = (double)gy / (hi - lo);
   AW_CUDA(launch_density(velocity_args(s), mode, s->status, s->n, hist_dev, gx, gy, lo, fx, fy,
                          reinterpret_cast<unsigned long long *>(dropped_dev), (cudaStream_t)s->stream));
   return AW_OK;
 }
+
+int aw_bound_energy(aw_state *s, void *scratch_dev) {
+  if (!s || !scratch_dev) return AW_EINVAL;
+  int rc = check_planes(s);
+  if (rc != AW_OK) return rc;
+  if (!aligned(scratch_dev, 8)) return AW_EINVAL;
+  if (!s->ready || !std::isfinite(s->eps)) return AW_ESTATE;
+  if (s->n == 0) return AW_OK;
+  cudaStream_t st = (cudaStream_t)s->stream;
+  unsigned long long key = 0ull;
+  AW_CUDA(cudaMemsetAsync(scratch_dev, 0, 8, st));
+  AW_CUDA(launch_energy_bound(s->q, s->status, s->n, s->pitch, s->eps, static_cast<unsigned long long *>(scratch_dev), st));
+  AW_CUDA(cudaMemcpyAsync(&key, scratch_dev, 8, cudaMemcpyDeviceToHost, st));
+  AW_CUDA(cudaStreamSynchronize(st));
+  bool any = false;
+  const double h = energy_key_decode(key, &any);
+  if (any) s->Emax = h;
+  return AW_OK;
+}
+
+}  // extern "C"
+
+// Both *_map_host calls: everything that can be checked without the data is checked before the first copy is
+// enqueued; once work is in flight every exit path synchronises the stream first (the header promises that the
+// caller's host buffers are free again when the call returns).
+namespace {
+int synced(cudaStream_t st, int rc) {
+  const cudaError_t e = cudaStreamSynchronize(st);
+  if (rc == AW_OK && e != cudaSuccess) return ::aw::cuda_fail(e);
+  return rc;
+}
+#define AW_CUDA_SYNCED(call)                                                      \
+  do {                                                                            \
+    cudaError_t e_ = (call);                                                      \
+    if (e_ != cudaSuccess) { cudaStreamSynchronize(st); return ::aw::cuda_fail(e_); } \
+  } while (0)
+
+int validate_integrate_args(const aw_state *s, int64_t steps, double dt, int64_t stride) {
+  if (steps < 0 || stride <= 0 || steps % stride != 0) return AW_EINVAL;
+  if (!(dt != 0.0) || !std::isfinite(dt)) return AW_EINVAL;
+  if (s->order != 4 && s->order != 6) return AW_ESTATE;
+  if (!std::isfinite(s->E) || !std::isfinite(s->eps)) return AW_ESTATE;
+  if (stride > 0x7fffffff) return AW_ERANGE;
+  if (s->survive != 0 && s->survive != 1) return AW_EINVAL;
+  if (s->survive && !(s->surv_hi_x > s->surv_lo_x && s->surv_hi_y > s->surv_lo_y)) return AW_EINVAL;
+  if (s->block != 0 && s->block != 32 && s->block != 64 && s->block != 128) return AW_EINVAL;
+  return AW_OK;
+}
+
+int validate_hist_args(int32_t gx, int32_t gy, double lo, double hi, const void *hist_dev) {
+  if (gx <= 0 || gy <= 0 || !(hi > lo) || !std::isfinite(lo) || !std::isfinite(hi)) return AW_EINVAL;
+  if ((int64_t)gx * gy >= 0xffffffffll) return AW_ERANGE;
+  if (!hist_dev || !aligned(hist_dev, 8)) return AW_EINVAL;
+  return AW_OK;
+}
+
+int upload_state(aw_state *s, const aw_host_in *in, cudaStream_t st) {
+  const size_t P = (size_t)s->pitch;
+  if (s->n == 0) return AW_OK;
+  AW_CUDA_SYNCED(cudaMemcpyAsync(s->q, in->q, 6 * P * 8, cudaMemcpyHostToDevice, st));
+  if (s->w) AW_CUDA_SYNCED(cudaMemcpyAsync(s->w, in->w, 6 * P * 8, cudaMemcpyHostToDevice, st));
+  AW_CUDA_SYNCED(cudaMemcpyAsync(s->acc, in->acc, 4 * P * 8, cudaMemcpyHostToDevice, st));
+  if (s->wind) AW_CUDA_SYNCED(cudaMemcpyAsync(s->wind, in->wind, 3 * P * 4, cudaMemcpyHostToDevice, st));
+  AW_CUDA_SYNCED(cudaMemcpyAsync(s->status, in->status, (size_t)s->n, cudaMemcpyHostToDevice, st));
+  return AW_OK;
+}
+
+int download_state(const aw_state *s, const aw_host_out *out, cudaStream_t st) {
+  const size_t P = (size_t)s->pitch;
+  if (s->n == 0) return AW_OK;
+  if (out->q) AW_CUDA_SYNCED(cudaMemcpyAsync(out->q, s->q, 6 * P * 8, cudaMemcpyDeviceToHost, st));
+  if (out->acc) AW_CUDA_SYNCED(cudaMemcpyAsync(out->acc, s->acc, 4 * P * 8, cudaMemcpyDeviceToHost, st));
+  if (out->status) AW_CUDA_SYNCED(cudaMemcpyAsync(out->status, s->status, (size_t)s->n, cudaMemcpyDeviceToHost, st));
+  return AW_OK;
+}
+}  // namespace
+
+extern "C" {
 
 int aw_map_host(aw_state *s, const aw_host_in *in, int64_t steps, double dt, int64_t stride, int kind,
                 double thr, int32_t gx, int32_t gy, double lo, double hi, void *ind_dev, void *hist_dev,
@@ -425,40 +531,40 @@ int aw_map_host(aw_state *s, const aw_host_in *in, int64_t steps, double dt, int
   int rc = check_planes(s);
   if (rc != AW_OK) return rc;
   if (!in->q || !in->acc || !in->status || (s->w && !in->w) || (s->wind && !in->wind)) return AW_EINVAL;
-  if (out->image && !ind_dev) return AW_EINVAL;
-  if (out->hist && !hist_dev) return AW_EINVAL;
+  if ((rc = validate_integrate_args(s, steps, dt, stride)) != AW_OK) return rc;
+  if (out->image) {  // what aw_indicator would refuse after the integration, refused now
+    if (!ind_dev) return AW_EINVAL;
+    if (kind < AW_IND_FLI || kind > AW_IND_DHS) return AW_EINVAL;
+    if (kind >= AW_IND_DP && kind <= AW_IND_VZ) return AW_ESTATE;  // need a snapshot: aw_velocity_map_host
+    if ((kind == AW_IND_FLI || kind == AW_IND_FTLE || kind == AW_IND_CLASS) && !s->w) return AW_ESTATE;
+    if (kind == AW_IND_FTLE && !(s->t + (double)steps * std::fabs(dt) > 0.0)) return AW_ESTATE;
+    if (kind == AW_IND_CLASS && thr != thr) return AW_EINVAL;
+    if (kind != AW_IND_CLASS && !aligned16(ind_dev)) return AW_EINVAL;
+  }
+  if (out->hist && (rc = validate_hist_args(gx, gy, lo, hi, hist_dev)) != AW_OK) return rc;
   cudaStream_t st = (cudaStream_t)s->stream;
-  const size_t P = (size_t)s->pitch;
-  // host -> device
-  AW_CUDA(cudaMemcpyAsync(s->q, in->q, 6 * P * 8, cudaMemcpyHostToDevice, st));
-  if (s->w) AW_CUDA(cudaMemcpyAsync(s->w, in->w, 6 * P * 8, cudaMemcpyHostToDevice, st));
-  AW_CUDA(cudaMemcpyAsync(s->acc, in->acc, 4 * P * 8, cudaMemcpyHostToDevice, st));
-  if (s->wind) AW_CUDA(cudaMemcpyAsync(s->wind, in->wind, 3 * P * 4, cudaMemcpyHostToDevice, st));
-  AW_CUDA(cudaMemcpyAsync(s->status, in->status, (size_t)s->n, cudaMemcpyHostToDevice, st));
+  if ((rc = upload_state(s, in, st)) != AW_OK) return rc;
   s->ready = 1;
-  rc = aw_integrate(s, s->n, steps, dt, stride);
-  if (rc != AW_OK) return rc;
+  // the trigonometry level from the uploaded data, not from the struct's E
+  void *scratch = (out->hist && hist_dev) ? hist_dev : (aligned(ind_dev, 8) ? ind_dev : nullptr);
+  if (scratch && (rc = aw_bound_energy(s, scratch)) != AW_OK) return synced(st, rc);
+  if ((rc = aw_integrate(s, s->n, steps, dt, stride)) != AW_OK) return synced(st, rc);
   if (out->image) {
-    rc = aw_indicator(s, kind, thr, ind_dev);
-    if (rc != AW_OK) return rc;
+    if ((rc = aw_indicator(s, kind, thr, ind_dev)) != AW_OK) return synced(st, rc);
     const size_t bytes = (kind == AW_IND_CLASS) ? (size_t)s->n : (size_t)s->n * 8;
-    AW_CUDA(cudaMemcpyAsync(out->image, ind_dev, bytes, cudaMemcpyDeviceToHost, st));
+    if (s->n > 0) AW_CUDA_SYNCED(cudaMemcpyAsync(out->image, ind_dev, bytes, cudaMemcpyDeviceToHost, st));
   }
   if (out->hist) {
-    const size_t hb = (size_t)gx * gy * 4;
-    if (gx <= 0 || gy <= 0) return AW_EINVAL;
-    AW_CUDA(cudaMemsetAsync(hist_dev, 0, hb + 8, st));
-    uint64_t *drop_dev = reinterpret_cast<uint64_t *>(static_cast<char *>(hist_dev) + hb);
-    rc = aw_density(s, static_cast<uint32_t *>(hist_dev), gx, gy, lo, hi, 0, drop_dev);
-    if (rc != AW_OK) return rc;
-    AW_CUDA(cudaMemcpyAsync(out->hist, hist_dev, hb, cudaMemcpyDeviceToHost, st));
-    if (out->dropped) AW_CUDA(cudaMemcpyAsync(out->dropped, drop_dev, 8, cudaMemcpyDeviceToHost, st));
+    const size_t hb = (size_t)gx * gy * 4, off = (hb + 7) / 8 * 8;  // counter 8-byte aligned for any gx*gy
+    AW_CUDA_SYNCED(cudaMemsetAsync(hist_dev, 0, off + 8, st));
+    uint64_t *drop_dev = reinterpret_cast<uint64_t *>(static_cast<char *>(hist_dev) + off);
+    if ((rc = aw_density(s, static_cast<uint32_t *>(hist_dev), gx, gy, lo, hi, 0, drop_dev)) != AW_OK)
+      return synced(st, rc);
+    AW_CUDA_SYNCED(cudaMemcpyAsync(out->hist, hist_dev, hb, cudaMemcpyDeviceToHost, st));
+    if (out->dropped) AW_CUDA_SYNCED(cudaMemcpyAsync(out->dropped, drop_dev, 8, cudaMemcpyDeviceToHost, st));
   }
-  if (out->q) AW_CUDA(cudaMemcpyAsync(out->q, s->q, 6 * P * 8, cudaMemcpyDeviceToHost, st));
-  if (out->acc) AW_CUDA(cudaMemcpyAsync(out->acc, s->acc, 4 * P * 8, cudaMemcpyDeviceToHost, st));
-  if (out->status) AW_CUDA(cudaMemcpyAsync(out->status, s->status, (size_t)s->n, cudaMemcpyDeviceToHost, st));
-  AW_CUDA(cudaStreamSynchronize(st));
-  return AW_OK;
+  if ((rc = download_state(s, out, st)) != AW_OK) return rc;
+  return synced(st, AW_OK);
 }
 
 int aw_velocity_map_host(aw_state *s, const aw_host_in *in, int64_t steps, double dt, int64_t stride, int mode,
@@ -467,109 +573,26 @@ int aw_velocity_map_host(aw_state *s, const aw_host_in *in, int64_t steps, doubl
   int rc = check_planes(s);
   if (rc != AW_OK) return rc;
   if (!in->q || !in->acc || !in->status || (s->w && !in->w) || (s->wind && !in->wind)) return AW_EINVAL;
-  if (mode < AW_DENS_VEL_UPPER || mode > AW_DENS_VEL_BOTH || gx <= 0 || gy <= 0) return AW_EINVAL;
-  if (s->n > 0 && !has_ref(s)) return AW_ESTATE;
+  if (mode < AW_DENS_VEL_UPPER || mode > AW_DENS_VEL_BOTH) return AW_EINVAL;
+  if ((rc = validate_hist_args(gx, gy, lo, hi, hist_dev)) != AW_OK) return rc;
+  if ((rc = validate_integrate_args(s, steps, dt, stride)) != AW_OK) return rc;
+  if (s->n > 0 && !has_velocity_ref(s)) return AW_ESTATE;
+  if (steps == 0) return AW_ESTATE;  // empty averaging window
   cudaStream_t st = (cudaStream_t)s->stream;
-  const size_t P = (size_t)s->pitch;
-  AW_CUDA(cudaMemcpyAsync(s->q, in->q, 6 * P * 8, cudaMemcpyHostToDevice, st));
-  if (s->w) AW_CUDA(cudaMemcpyAsync(s->w, in->w, 6 * P * 8, cudaMemcpyHostToDevice, st));
-  AW_CUDA(cudaMemcpyAsync(s->acc, in->acc, 4 * P * 8, cudaMemcpyHostToDevice, st));
-  if (s->wind) AW_CUDA(cudaMemcpyAsync(s->wind, in->wind, 3 * P * 4, cudaMemcpyHostToDevice, st));
-  AW_CUDA(cudaMemcpyAsync(s->status, in->status, (size_t)s->n, cudaMemcpyHostToDevice, st));
+  if ((rc = upload_state(s, in, st)) != AW_OK) return rc;
   s->ready = 1;
-  rc = aw_mark(s);
-  if (rc != AW_OK) return rc;
-  rc = aw_integrate(s, s->n, steps, dt, stride);
-  if (rc != AW_OK) return rc;
-  const size_t hb = (size_t)gx * gy * 4;
-  AW_CUDA(cudaMemsetAsync(hist_dev, 0, hb + 8, st));
-  uint64_t *drop_dev = reinterpret_cast<uint64_t *>(static_cast<char *>(hist_dev) + hb);
-  rc = aw_density(s, static_cast<uint32_t *>(hist_dev), gx, gy, lo, hi, mode, drop_dev);
-  if (rc != AW_OK) return rc;
-  AW_CUDA(cudaMemcpyAsync(out->hist, hist_dev, hb, cudaMemcpyDeviceToHost, st));
-  if (out->dropped) AW_CUDA(cudaMemcpyAsync(out->dropped, drop_dev, 8, cudaMemcpyDeviceToHost, st));
-  if (out->q) AW_CUDA(cudaMemcpyAsync(out->q, s->q, 6 * P * 8, cudaMemcpyDeviceToHost, st));
-  if (out->acc) AW_CUDA(cudaMemcpyAsync(out->acc, s->acc, 4 * P * 8, cudaMemcpyDeviceToHost, st));
-  if (out->status) AW_CUDA(cudaMemcpyAsync(out->status, s->status, (size_t)s->n, cudaMemcpyDeviceToHost, st));
-  AW_CUDA(cudaStreamSynchronize(st));
-  return AW_OK;
-}
-
-int aw_sincos_probe(const double *x_dev, int64_t n, double *sin_dev, double *cos_dev, void *stream) {
-  if (!x_dev || !sin_dev || !cos_dev || n < 0) return AW_EINVAL;
-  if (n == 0) return AW_OK;
-  AW_CUDA(launch_sincos_probe(x_dev, n, sin_dev, cos_dev, (cudaStream_t)stream));
-  AW_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
-  return AW_OK;
-}
-
-int aw_uniform_probe(uint64_t seed, uint64_t k0, int64_t n, uint32_t slot, double *out_dev, void *stream) {
-  if (!out_dev || n < 0 || slot > 15) return AW_EINVAL;
-  if (n == 0) return AW_OK;
-  AW_CUDA(launch_uniform_probe(seed, k0, n, slot, out_dev, (cudaStream_t)stream));
-  AW_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
-  return AW_OK;
-}
-
-int aw_hamiltonian_probe(const double *q_dev, int64_t n, int64_t pitch, double eps, double *out_dev,
-                         void *stream) {
-  if (!q_dev || !out_dev || n < 0 || pitch < n) return AW_EINVAL;
-  if (n == 0) return AW_OK;
-  AW_CUDA(launch_hamiltonian_probe(q_dev, n, pitch, eps, out_dev, (cudaStream_t)stream));
-  AW_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
-  return AW_OK;
-}
-
-int aw_dfma_peak_probe(int blocks, int threads, int chains, int64_t iters, double *sink_dev,
-                       double *ms_host, double *dfma_host, void *stream) {
-  if (blocks <= 0 || threads <= 0 || threads > 1024 || iters <= 0 || !sink_dev || !ms_host || !dfma_host)
-    return AW_EINVAL;
-  if (chains != 1 && chains != 2 && chains != 4 && chains != 8 && chains != 16) return AW_EINVAL;
-  iters = (iters + 7) / 8 * 8;
-  cudaStream_t st = (cudaStream_t)stream;
-  cudaEvent_t e0, e1;
-  AW_CUDA(cudaEventCreate(&e0));
-  AW_CUDA(cudaEventCreate(&e1));
-  cudaError_t err = launch_dfma_peak(blocks, threads, chains, iters / 8 > 16 ? 128 : iters, sink_dev, st);  // warm-up
-  if (err == cudaSuccess) err = cudaEventRecord(e0, st);
-  if (err == cudaSuccess) err = launch_dfma_peak(blocks, threads, chains, iters, sink_dev, st);
-  if (err == cudaSuccess) err = cudaEventRecord(e1, st);
-  if (err == cudaSuccess) err = cudaEventSynchronize(e1);
-  float ms = 0.f;
-  if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  if (err != cudaSuccess) return cuda_fail(err);
-  *ms_host = (double)ms;
-  *dfma_host = (double)blocks * (double)threads * (double)chains * (double)iters;
-  return AW_OK;
-}
-
-int aw_dfma_shape_probe(int blocks, int threads, int shape, int64_t iters, double *work_dev, double *ms_host,
-                        double *inst_host, void *stream) {
-  if (blocks <= 0 || threads <= 0 || threads > 1024 || iters <= 0 || !work_dev || !ms_host || !inst_host)
-    return AW_EINVAL;
-  if (shape < 0 || shape > 5) return AW_EINVAL;
-  cudaStream_t st = (cudaStream_t)stream;
-  double host[128];
-  for (int i = 0; i < 128; ++i) host[i] = 1.0 - 1e-9 * (double)(i % 97);
-  AW_CUDA(cudaMemcpyAsync(work_dev, host, sizeof host, cudaMemcpyHostToDevice, st));
-  cudaEvent_t e0, e1;
-  AW_CUDA(cudaEventCreate(&e0));
-  AW_CUDA(cudaEventCreate(&e1));
-  cudaError_t err = launch_dfma_shape(blocks, threads, shape, 64, work_dev + 128, work_dev, st);  // warm-up
-  if (err == cudaSuccess) err = cudaEventRecord(e0, st);
-  if (err == cudaSuccess) err = launch_dfma_shape(blocks, threads, shape, iters, work_dev + 128, work_dev, st);
-  if (err == cudaSuccess) err = cudaEventRecord(e1, st);
-  if (err == cudaSuccess) err = cudaEventSynchronize(e1);
-  float ms = 0.f;
-  if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  if (err != cudaSuccess) return cuda_fail(err);
-  *ms_host = (double)ms;
-  *inst_host = (double)blocks * (double)threads * (double)iters * 32.0;
-  return AW_OK;
+  if ((rc = aw_bound_energy(s, hist_dev)) != AW_OK) return synced(st, rc);
+  if ((rc = aw_mark(s)) != AW_OK) return synced(st, rc);
+  if ((rc = aw_integrate(s, s->n, steps, dt, stride)) != AW_OK) return synced(st, rc);
+  const size_t hb = (size_t)gx * gy * 4, off = (hb + 7) / 8 * 8;
+  AW_CUDA_SYNCED(cudaMemsetAsync(hist_dev, 0, off + 8, st));
+  uint64_t *drop_dev = reinterpret_cast<uint64_t *>(static_cast<char *>(hist_dev) + off);
+  if ((rc = aw_density(s, static_cast<uint32_t *>(hist_dev), gx, gy, lo, hi, mode, drop_dev)) != AW_OK)
+    return synced(st, rc);
+  AW_CUDA_SYNCED(cudaMemcpyAsync(out->hist, hist_dev, hb, cudaMemcpyDeviceToHost, st));
+  if (out->dropped) AW_CUDA_SYNCED(cudaMemcpyAsync(out->dropped, drop_dev, 8, cudaMemcpyDeviceToHost, st));
+  if ((rc = download_state(s, out, st)) != AW_OK) return rc;
+  return synced(st, AW_OK);
 }
 
 }  // extern "C"

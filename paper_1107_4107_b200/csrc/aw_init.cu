@@ -28,8 +28,10 @@ __global__ void __launch_bounds__(256) init_shell_kernel(const __grid_constant__
   if (k >= p.n) return;
   const int64_t P = p.pitch;
   const aw_grid &g = p.g;
-  const int64_t i = k % g.gx, j = k / g.gx;
-  const uint64_t uk = (uint64_t)k;
+  // K: index in the whole ensemble the grid describes (grid position, random-number counter); k: slot in the planes
+  const int64_t K = g.k0 + k;
+  const int64_t i = K % g.gx, j = K / g.gx;
+  const uint64_t uk = (uint64_t)K;
 
   double x = 0.0, y = 0.0, z = 0.0;
   if (g.angle_mode == 1) {
@@ -104,38 +106,10 @@ __global__ void __launch_bounds__(256) init_shell_kernel(const __grid_constant__
   }
 }
 
-__global__ void uniform_probe_kernel(uint64_t seed, uint64_t k0, int64_t n, uint32_t slot, double *out) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) out[i] = uniform01(seed, k0 + (uint64_t)i, slot);
-}
-
-__global__ void sincos_probe_kernel(const double *x, int64_t n, double *s, double *c) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) {
-    double sn, cs;
-    sincos(x[i], sn, cs);
-    s[i] = sn;
-    c[i] = cs;
-  }
-}
-
 }  // namespace
 
 cudaError_t launch_init(const InitParams &p, cudaStream_t st) {
   init_shell_kernel<<<(unsigned)((p.n + 255) / 256), 256, 0, st>>>(p);
-  count_launch();
-  return cudaGetLastError();
-}
-
-cudaError_t launch_uniform_probe(uint64_t seed, uint64_t k0, int64_t n, uint32_t slot, double *out,
-                                 cudaStream_t st) {
-  uniform_probe_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(seed, k0, n, slot, out);
-  count_launch();
-  return cudaGetLastError();
-}
-
-cudaError_t launch_sincos_probe(const double *x, int64_t n, double *s, double *c, cudaStream_t st) {
-  sincos_probe_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(x, n, s, c);
   count_launch();
   return cudaGetLastError();
 }

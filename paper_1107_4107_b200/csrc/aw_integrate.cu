@@ -272,7 +272,8 @@ __device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p) {
 template <int S, bool TAN, int LEVEL>
 __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS(LEVEL))
     integrate_kernel(const __grid_constant__ IntegrateParams p) {
-  const int64_t k = (int64_t)blockIdx.x * AW_BLOCK + threadIdx.x;
+  // blocks of 32, 64 or 128 threads (launch_one): the arithmetic is per trajectory, so the result does not depend on it
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= p.n) return;
   if (p.status[k] != AW_ST_LIVE) return;
   const int64_t P = p.pitch;
@@ -349,8 +350,9 @@ __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS(LEVEL))
 
 template <int S, bool TAN, int LEVEL>
 cudaError_t launch_one(const IntegrateParams &p, cudaStream_t st) {
-  const int64_t blocks = (p.n + AW_BLOCK - 1) / AW_BLOCK;
-  integrate_kernel<S, TAN, LEVEL><<<(unsigned)blocks, AW_BLOCK, 0, st>>>(p);
+  const int block = p.block;
+  const int64_t blocks = (p.n + block - 1) / block;
+  integrate_kernel<S, TAN, LEVEL><<<(unsigned)blocks, block, 0, st>>>(p);
   count_launch();
   return cudaGetLastError();
 }
@@ -403,6 +405,29 @@ int trig_level_for(double d) {
   return 0;
 }
 
+double trig_level_max_angle(int level) {
+  return (level >= 1 && level <= 9) ? kLevelMaxD[level] : INFINITY;
+}
+
+// Threads per block from the ensemble size: 128 (the tuned shape) once that fills every SM with its
+// 4 resident blocks; smaller ensembles get 64- or 32-thread blocks so that their warps spread over all SMs (and
+// over the four sub-partitions of each) instead of piling 4 warps on a quarter of the chip.
+int integrate_block_size(int64_t n, int forced) {
+  if (forced == 32 || forced == 64 || forced == 128) return forced;
+  static int sms[64] = {0};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) dev = 0;
+  if (sms[dev] == 0) {
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) v = 148;
+    sms[dev] = v;
+  }
+  const int64_t full = (int64_t)sms[dev] * 4;   // blocks of one full wave at 4 resident 128-thread blocks per SM
+  if ((n + 127) / 128 >= full) return 128;
+  if ((n + 63) / 64 >= full) return 64;
+  return 32;
+}
+
 // The per-drift degrees assume the ratios |a_loop[cs]| / max |a_loop| of the two built-in stage lists.
 bool drift_ratios_hold(int S, const double *a_loop) {
   double amax = 0.0;
@@ -420,18 +445,6 @@ cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, 
   if (p.level >= 1 && p.level <= 7) return launch_integrate_low(p, order, tangent, st);
   if (order == 4) return tangent ? launch_level<3, true>(p, st) : launch_level<3, false>(p, st);
   return tangent ? launch_level<7, true>(p, st) : launch_level<7, false>(p, st);
-}
-
-__global__ void hamiltonian_probe_kernel(const double *q, int64_t n, int64_t P, double eps, double *out) {
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k < n) out[k] = hamiltonian_dev(q[k], q[P + k], q[2 * P + k], q[3 * P + k], q[4 * P + k], q[5 * P + k], eps);
-}
-
-cudaError_t launch_hamiltonian_probe(const double *q, int64_t n, int64_t pitch, double eps, double *out,
-                                     cudaStream_t st) {
-  hamiltonian_probe_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(q, n, pitch, eps, out);
-  count_launch();
-  return cudaGetLastError();
 }
 
 #endif  // AW_LEVEL_GROUP

@@ -38,6 +38,7 @@ struct IntegrateParams {
   double b2[kMaxStages];     // 2 b_s
   double eps;
   int32_t survive;  // survivor filter (R25): 1 = test (px, py) against surv[] at every checkpoint
+  int32_t block;    // threads per block (32, 64 or 128)
   double surv[4];   // lo_x, hi_x, lo_y, hi_y (half-open)
 };
 
@@ -58,6 +59,9 @@ struct InitParams {
 cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, cudaStream_t st);
 // Trigonometry variant for a largest drift angle max_s |a_s| * max|p| (0 = full sincos every stage).
 int trig_level_for(double max_drift_angle);
+// largest drift angle max_s |a_s| * max|p| the level supports (infinity for level 0)
+double trig_level_max_angle(int level);
+int integrate_block_size(int64_t n, int forced);
 // true if |a_loop[s]| / max |a_loop| are within the ratios the per-drift Taylor degrees were derived for
 bool drift_ratios_hold(int S, const double *a_loop);
 constexpr int kMaxChunk = 128;
@@ -79,22 +83,19 @@ cudaError_t launch_indicator_ref(const VelocityArgs &v, const uint8_t *status, i
 cudaError_t launch_density(const VelocityArgs &v, int mode, const uint8_t *status, int64_t n,
                            uint32_t *hist, int32_t gx, int32_t gy, double lo, double fx, double fy,
                            unsigned long long *dropped, cudaStream_t st);
-cudaError_t launch_sincos_probe(const double *x, int64_t n, double *s, double *c, cudaStream_t st);
-cudaError_t launch_uniform_probe(uint64_t seed, uint64_t k0, int64_t n, uint32_t slot, double *out,
-                                 cudaStream_t st);
-cudaError_t launch_hamiltonian_probe(const double *q, int64_t n, int64_t pitch, double eps, double *out,
-                                     cudaStream_t st);
-cudaError_t launch_dfma_peak(int blocks, int threads, int chains, int64_t iters, double *sink,
-                             cudaStream_t st);
-
 int64_t energy_stats_blocks(int64_t n);
 size_t energy_partial_bytes();
 cudaError_t launch_energy_stats(const double *q, const double *acc, const uint8_t *status, int64_t n, int64_t pitch,
                                 double eps, void *scratch, double *out, cudaStream_t st);
 cudaError_t launch_signed_dh(const double *q, const double *acc, const uint8_t *status, int64_t n, int64_t pitch,
                              double eps, double *out, cudaStream_t st);
-cudaError_t launch_dfma_shape(int blocks, int threads, int shape, int64_t iters, double *sink, const double *in,
-                              cudaStream_t st);
+// max over live, finite trajectories of H(X,P), as a monotone 64-bit key (0 = none) in *key_out (aw_bound_energy)
+cudaError_t launch_energy_bound(const double *q, const uint8_t *status, int64_t n, int64_t pitch, double eps,
+                                unsigned long long *key_out, cudaStream_t st);
+double energy_key_decode(unsigned long long key, bool *any);
+// status <- AW_ST_RANGE where a live trajectory's H(X,P) exceeds hmax (the precondition of the integrator's arithmetic)
+cudaError_t launch_range_check(const double *q, uint8_t *status, int64_t n, int64_t pitch, double eps, double hmax,
+                               cudaStream_t st);
 
 void count_launch();
 

@@ -1,4 +1,6 @@
 // aw_reduce.cu — §8(a) a5 (indicator image) and a6 (visited-cell density histogram); DESIGN.md §6.3-6.4.
+#include <cstring>
+
 #include "aw_internal.cuh"
 #include "aw_model.cuh"
 
@@ -256,81 +258,52 @@ __global__ void __launch_bounds__(kDensityBlock)
   if (threadIdx.x == 0 && dropped && block_dropped) atomicAdd(dropped, (unsigned long long)block_dropped);
 }
 
-// ------------------------------------------------------------------------------- fp64 peak probe
-template <int CH>
-__global__ void dfma_peak_kernel(int64_t iters, double *sink) {
-  double v[CH];
-  const double a = 1.0 - 1e-9 * (double)(threadIdx.x & 7), b = 1e-12;
-#pragma unroll
-  for (int c = 0; c < CH; ++c) v[c] = (double)(threadIdx.x + c);
-#pragma unroll 1
-  for (int64_t i = 0; i < iters; i += 8) {
-#pragma unroll
-    for (int u = 0; u < 8; ++u) {
-#pragma unroll
-      for (int c = 0; c < CH; ++c) v[c] = fma(v[c], a, b);
-    }
-  }
-  double acc = 0.0;
-#pragma unroll
-  for (int c = 0; c < CH; ++c) acc += v[c];
-  if (acc == 123.456) sink[0] = acc;  // never true in practice; keeps the chains alive
+// ------------------------------------------------------------------------------- precondition of aw_integrate
+// Enforced, not assumed (include/aw.h, aw_state.Emax): P^2 <= 2(H + 2|eps|) on the whole orbit, so the largest
+// drift angle of a trajectory is bounded by its energy; one whose energy exceeds what the Taylor degrees of the chosen
+// trigonometry level (and the angle range of R7) were sized for is flagged AW_ST_RANGE before the integrator runs
+// and is never touched.  A non-finite H is the checkpoint's business (status 2).  Runs once per aw_integrate call:
+// 49 bytes per trajectory, HBM bound, ~1e-4 of a 20 000-step launch.
+__global__ void __launch_bounds__(256) range_check_kernel(const double *__restrict__ q, uint8_t *__restrict__ status,
+                                                          int64_t n, int64_t P, double eps, double hmax) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n || status[k] != AW_ST_LIVE) return;
+  const double h = hamiltonian_dev(q[k], q[P + k], q[2 * P + k], q[3 * P + k], q[4 * P + k], q[5 * P + k], eps);
+  if (h > hmax && h <= 1.7976931348623157e308) status[k] = (uint8_t)AW_ST_RANGE;
 }
 
-// fp64 issue rate by operand shape: 8 independent chains per thread, 32 instructions per loop trip.
-//   0: fma(v, u0, w0)    three registers, two of them shared by neighbouring instructions (reuse cache)
-//   1: fma(v, u_c, w_c)  three distinct registers, nothing shared with the neighbours
-//   2: fma(v, u_c, imm)  two registers + an immediate
-//   3: fma(v, v, w_c)    three register operands, two distinct
-//   4: v * u_c           DMUL, two registers
-//   5: fma(u_c, w_c', v) accumulate form, three distinct registers
-template <int SHAPE>
-__global__ void dfma_shape_kernel(int64_t iters, double *sink, const double *in) {
-  constexpr int CH = 8;
-  double v[CH], u[CH], w[CH];
-#pragma unroll
-  for (int c = 0; c < CH; ++c) {
-    v[c] = in[(threadIdx.x + c) & 127];
-    u[c] = in[(threadIdx.x + 32 + c) & 127];
-    w[c] = in[(threadIdx.x + 64 + c) & 127];
+// ------------------------------------------------------------------------------- aw_bound_energy
+// max over live trajectories of H(X,P) (finite values only): doubles map to 64-bit keys whose unsigned order is the
+// numeric order, so one atomicMax per block on an 8-byte scratch word gives an order-independent, exact maximum.
+__device__ __forceinline__ unsigned long long energy_key(double h) {
+  const unsigned long long b = (unsigned long long)__double_as_longlong(h);
+  return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+
+__global__ void __launch_bounds__(256) energy_bound_kernel(const double *__restrict__ q,
+                                                           const uint8_t *__restrict__ status, int64_t n, int64_t P,
+                                                           double eps, unsigned long long *key_out) {
+  __shared__ unsigned long long sh[8];
+  unsigned long long key = 0ull;
+  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+    if (status[k] != AW_ST_LIVE) continue;
+    const double h = hamiltonian_dev(q[k], q[P + k], q[2 * P + k], q[3 * P + k], q[4 * P + k], q[5 * P + k], eps);
+    if (isfinite(h)) { const unsigned long long kk = energy_key(h); key = kk > key ? kk : key; }
   }
-#pragma unroll 1
-  for (int64_t i = 0; i < iters; ++i) {
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-#pragma unroll
-      for (int c = 0; c < CH; ++c) {
-        if (SHAPE == 0) v[c] = fma(v[c], u[0], w[0]);
-        if (SHAPE == 1) v[c] = fma(v[c], u[c], w[c]);
-        if (SHAPE == 2) v[c] = fma(v[c], u[c], 1e-12);
-        if (SHAPE == 3) v[c] = fma(v[c], v[c], w[c]);
-        if (SHAPE == 4) v[c] = v[c] * u[c];
-        if (SHAPE == 5) v[c] = fma(u[c], w[(c + 1) % CH], v[c]);
-      }
-    }
+  for (int off = 16; off > 0; off >>= 1) {
+    const unsigned long long o = __shfl_down_sync(0xffffffffu, key, off);
+    key = o > key ? o : key;
   }
-  double acc = 0.0;
-#pragma unroll
-  for (int c = 0; c < CH; ++c) acc += v[c];
-  if (acc == 123.456) sink[0] = acc;
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = key;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) key = sh[w] > key ? sh[w] : key;
+    if (key) atomicMax(key_out, key);
+  }
 }
 
 }  // namespace
-
-cudaError_t launch_dfma_shape(int blocks, int threads, int shape, int64_t iters, double *sink, const double *in,
-                              cudaStream_t st) {
-  switch (shape) {
-    case 0: dfma_shape_kernel<0><<<blocks, threads, 0, st>>>(iters, sink, in); break;
-    case 1: dfma_shape_kernel<1><<<blocks, threads, 0, st>>>(iters, sink, in); break;
-    case 2: dfma_shape_kernel<2><<<blocks, threads, 0, st>>>(iters, sink, in); break;
-    case 3: dfma_shape_kernel<3><<<blocks, threads, 0, st>>>(iters, sink, in); break;
-    case 4: dfma_shape_kernel<4><<<blocks, threads, 0, st>>>(iters, sink, in); break;
-    case 5: dfma_shape_kernel<5><<<blocks, threads, 0, st>>>(iters, sink, in); break;
-    default: return cudaErrorInvalidValue;
-  }
-  count_launch();
-  return cudaGetLastError();
-}
 
 cudaError_t launch_indicator(const double *acc, const uint8_t *status, int64_t n, int64_t pitch, int kind,
                              double thr, double t, void *out, cudaStream_t st) {
@@ -385,18 +358,29 @@ cudaError_t launch_density(const VelocityArgs &v, int mode, const uint8_t *statu
   return cudaGetLastError();
 }
 
-cudaError_t launch_dfma_peak(int blocks, int threads, int chains, int64_t iters, double *sink,
-                             cudaStream_t st) {
-  switch (chains) {
-    case 1: dfma_peak_kernel<1><<<blocks, threads, 0, st>>>(iters, sink); break;
-    case 2: dfma_peak_kernel<2><<<blocks, threads, 0, st>>>(iters, sink); break;
-    case 4: dfma_peak_kernel<4><<<blocks, threads, 0, st>>>(iters, sink); break;
-    case 8: dfma_peak_kernel<8><<<blocks, threads, 0, st>>>(iters, sink); break;
-    case 16: dfma_peak_kernel<16><<<blocks, threads, 0, st>>>(iters, sink); break;
-    default: return cudaErrorInvalidValue;
-  }
+cudaError_t launch_range_check(const double *q, uint8_t *status, int64_t n, int64_t pitch, double eps, double hmax,
+                               cudaStream_t st) {
+  range_check_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(q, status, n, pitch, eps, hmax);
   count_launch();
   return cudaGetLastError();
+}
+
+cudaError_t launch_energy_bound(const double *q, const uint8_t *status, int64_t n, int64_t pitch, double eps,
+                                unsigned long long *key_out, cudaStream_t st) {
+  int64_t blocks = (n + 255) / 256;
+  if (blocks > 148 * 8) blocks = 148 * 8;
+  energy_bound_kernel<<<(unsigned)blocks, 256, 0, st>>>(q, status, n, pitch, eps, key_out);
+  count_launch();
+  return cudaGetLastError();
+}
+
+double energy_key_decode(unsigned long long key, bool *any) {
+  *any = key != 0ull;
+  const unsigned long long b = (key >> 63) ? (key & 0x7fffffffffffffffull) : ~key;
+  double h;
+  static_assert(sizeof h == sizeof b, "fp64");
+  memcpy(&h, &b, sizeof h);
+  return h;
 }
 
 }  // namespace aw

@@ -6,14 +6,16 @@ so the roofline fraction cannot be inflated by the accounting convention.  "Exec
 (all stages unrolled), so its DFMA / DMUL / DADD counts are the per-step counts (checkpoint and
 re-synchronisation code, < 1 % at stride 100, is outside that loop and not counted).
 
-    python -m paper_1107_4107_b200.sass_count          # table for every instantiation
+    python sass_count.py          # table for every instantiation
+
+Measurement support for bench.py (it needs cuobjdump); not part of the product package.
 """
 import collections
 import os
 import re
 import subprocess
 
-from .build import LIB
+from paper_1107_4107_b200.build import LIB
 
 _cache = {}
 

@@ -31,8 +31,21 @@ def test_library_exports_every_declared_symbol(aw):
     L = C.CDLL(os.path.join(ROOT, "paper_1107_4107_b200", "libaw.so"))
     for n in names:
         assert hasattr(L, n), n
-    assert aw.aw_version() == 120
+    assert aw.aw_version() == 200
+    assert not any("probe" in n for n in names)            # probes live in tests/libaw_probe.so, not in the product ABI
     assert aw.aw_strerror(0) == "ok" and "invalid" in aw.aw_strerror(-1)
+
+
+def test_probe_library_exports_its_header():
+    """tests/aw_probe.h (test and measurement support) is a separate library built from the same device headers."""
+    import aw_probe
+    src = open(os.path.join(ROOT, "tests", "aw_probe.h")).read()
+    names = sorted(set(re.findall(r"AWP_API\s+[\w\s\*]+?\b(awp_\w+)\s*\(", src)))
+    assert names == ["awp_dfma_peak", "awp_dfma_shape", "awp_hamiltonian", "awp_sincos", "awp_uniform"]
+    L = C.CDLL(aw_probe.build())
+    for n in names:
+        assert hasattr(L, n), n
+    assert L.awp_sincos(None, 4, None, None, None) == -1             # host-side validation, no device needed
 
 
 def test_python_binding_has_the_same_names(aw):
@@ -117,7 +130,12 @@ def test_validation_happens_on_the_host(aw):
     # init_shell
     assert L.aw_init_shell(C.byref(st), C.byref(g), 1.0, 0.6, 0) == ERANGE  # E - 2|eps| <= 0
     g.gx = 7
-    assert L.aw_init_shell(C.byref(st), C.byref(g), 1.0, 1e-2, 0) == EINVAL  # n != gx*gy
+    assert L.aw_init_shell(C.byref(st), C.byref(g), 1.0, 1e-2, 0) == EINVAL  # n > gx*gy: slice outside the ensemble
+    g.gx, g.k0 = 8, 1
+    assert L.aw_init_shell(C.byref(st), C.byref(g), 1.0, 1e-2, 0) == EINVAL  # k0 + n > gx*gy
+    g.k0 = -1
+    assert L.aw_init_shell(C.byref(st), C.byref(g), 1.0, 1e-2, 0) == EINVAL  # k0 < 0
+    g.k0 = 0
     g.gx, g.hi_x = 8, -1.0
     assert L.aw_init_shell(C.byref(st), C.byref(g), 1.0, 1e-2, 0) == EINVAL  # hi <= lo
     g.hi_x, g.shape = 1.0, 7
@@ -136,7 +154,46 @@ def test_validation_happens_on_the_host(aw):
     st.tref, st.t = 0.0, 0.0
     assert L.aw_density(C.byref(st), base, 16, 16, -1.0, 1.0, 1, None) == ESTATE   # empty window t == tref
     assert L.aw_indicator(C.byref(st), 5, 0.0, base) == ESTATE
-    st.qref = None
+    # the averaged velocity needs the turn counters as well (a wrapped angle without its count would alias silently)
+    st.t = 1.0
+    assert st.wind is None
+    assert L.aw_density(C.byref(st), base, 16, 16, -1.0, 1.0, 3, None) == ESTATE
+    assert L.aw_indicator(C.byref(st), 6, 0.0, base) == ESTATE
+    st.t, st.qref = 0.0, None
+    # histogram / drop-counter alignment (uint32 / uint64 atomics)
+    assert L.aw_density(C.byref(st), base + 2, 16, 16, -1.0, 1.0, 0, None) == EINVAL
+    assert L.aw_density(C.byref(st), base, 16, 16, -1.0, 1.0, 0, base + 4) == EINVAL
+    # block size: 0 (auto), 32, 64, 128
+    st.block = 48
+    assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == EINVAL
+    st.block = 0
+    # Emax raises the energy bound the trig level (and the R7 range) is sized for; below E it is ignored
+    st.Emax = 0.0
+    assert lv(0.005) == 1
+    st.Emax = 9.0
+    assert lv(0.005) == 3 and L.aw_integrate(C.byref(st), 64, 300, 1.0, 300) == ERANGE
+    st.Emax = float("nan")
+    assert lv(0.005) == 1 and L.aw_integrate(C.byref(st), 64, 0, 1.0, 300) == 0
+    st.Emax = 0.0
+    assert L.aw_bound_energy(C.byref(st), None) == EINVAL
+    assert L.aw_bound_energy(C.byref(st), base + 4) == EINVAL
+    # aw_map_host / aw_velocity_map_host: everything is refused BEFORE the first copy is enqueued
+    from paper_1107_4107_b200.binding import HostIn, HostOut
+    hin = HostIn(base, None, base, None, base)
+    hout = HostOut(base, base, None, None, None, None)
+    mh = lambda *a: L.aw_map_host(C.byref(st), C.byref(hin), *a, C.byref(hout))
+    assert mh(150, 0.01, 100, 2, 0.0, 16, 16, -1.0, 1.0, base, base) == EINVAL      # steps % stride
+    assert mh(100, 0.01, 100, 12, 0.0, 16, 16, -1.0, 1.0, base, base) == EINVAL     # no such indicator kind
+    assert mh(100, 0.01, 100, 0, 0.0, 16, 16, -1.0, 1.0, base, base) == ESTATE      # FLI without tangent planes
+    assert mh(100, 0.01, 100, 5, 0.0, 16, 16, -1.0, 1.0, base, base) == ESTATE      # velocity kinds need a snapshot
+    assert mh(100, 0.01, 100, 2, 0.0, 0, 16, -1.0, 1.0, base, base) == EINVAL       # gx <= 0
+    assert mh(100, 0.01, 100, 2, 0.0, 16, 16, 1.0, -1.0, base, base) == EINVAL      # hi <= lo
+    assert mh(100, 0.01, 100, 2, 0.0, 16, 16, -1.0, 1.0, None, base) == EINVAL      # image wanted, no scratch
+    assert mh(100, 0.01, 100, 2, 0.0, 16, 16, -1.0, 1.0, base, base + 4) == EINVAL  # histogram scratch misaligned
+    vm = lambda *a: L.aw_velocity_map_host(C.byref(st), C.byref(hin), *a, C.byref(hout))
+    assert vm(100, 0.01, 100, 0, 16, 16, -1.0, 1.0, base) == EINVAL                 # mode 0 is not a velocity mode
+    assert vm(100, 0.01, 100, 1, 16, 16, -1.0, 1.0, base) == ESTATE                 # no snapshot / counter planes
+    assert vm(100, 0.01, 100, 1, 16, 0, -1.0, 1.0, base) == EINVAL
     # survivor filter: flag must be 0/1 and the rectangle non-empty
     st.survive = 2
     assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == EINVAL

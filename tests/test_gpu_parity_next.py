@@ -61,7 +61,29 @@ def test_sphere_init_matches_oracle_generator(aw, orc, E, eps, pz_sign):
 
 # ------------------------------------------------------------------ P:67 averaged velocity, density on S
 
-@pytest.mark.parametrize("wind", [True, False])
+def test_velocity_needs_the_turn_counters(aw):
+    """Without wind / windref planes the averaged velocity is refused (AW_ESTATE): the checkpoint wraps the angles
+    whether or not the turns are counted, so a window with a completed turn would alias silently.  dP (momenta only)
+    and aw_mark still work."""
+    n = 64
+    ens = aw.Ensemble(n, tangent=False, wind=False, ref=True)
+    aw.aw_init_shell(ens, aw.make_grid(8, 8, angle_mode=1), 1.0, 1e-2, 1)
+    aw.aw_mark(ens)
+    aw.aw_integrate(ens, n, 100, 0.01, 100)
+    hist = torch.zeros((8, 8), dtype=torch.int32, device="cuda")
+    for mode in (1, 2, 3):
+        with pytest.raises(aw.AwError) as ei:
+            aw.aw_density(ens, hist, -2.0, 2.0, mode)
+        assert ei.value.code == -4
+    for kind in (aw.AW_IND_VX, aw.AW_IND_VY, aw.AW_IND_VZ):
+        with pytest.raises(aw.AwError) as ei:
+            aw.aw_indicator(ens, kind)
+        assert ei.value.code == -4
+    assert bool(torch.isfinite(aw.aw_indicator(ens, aw.AW_IND_DP)).all())
+    assert int(hist.sum().item()) == 0
+
+
+@pytest.mark.parametrize("wind", [True])
 def test_velocity_indicators_and_density_bit_exact(aw, orc, wind):
     """mark -> integrate -> (V, Vhat, dP, density on the sphere) from the SAME device state on both sides:
     bit-equal doubles, bit-exact counts, in every hemisphere mode, ragged size, accumulated twice."""
