@@ -262,6 +262,9 @@ struct awo_grid {
   int32_t tangent_mode;  // 0: one common seeded unit vector; 1: per trajectory
   int64_t k0;            // the state holds trajectories [k0, k0 + n) of the gx*gy ensemble the grid describes
                          // (independent realisations, so any contiguous slice can be generated alone)
+  int32_t resample;      // cloud shapes 1, 2: redraw a trajectory whose (px, py, X) has no real v_z, up to this many
+                         // times (R31); 0: mask it (status 0, R8)
+  int32_t reserved_;
 };
 
 double awo_hp(double x, double y, double z) { return Hp(x, y, z); }
@@ -303,50 +306,60 @@ int awo_init_shell(const awo_grid *g, double E, double eps, uint64_t seed, int64
     // K: index in the whole ensemble (grid position and random-number counter); k: slot in this state's planes
     const int64_t K = g->k0 + k;
     const int64_t i = K % g->gx, j = K / g->gx;
-    double X[3] = {0.0, 0.0, 0.0};
-    if (g->angle_mode == 1)
-      for (int al = 0; al < 3; ++al) X[al] = TWO_PI_HI * uniform01(seed, (uint64_t)K, (uint64_t)al);
     double st[6];
-    if (g->shape == 3) {
-      // P:85 "initial conditions uniformly distributed over the sphere S": direction uniform on the unit
-      // sphere (cos(theta) = 1 - 2 u3 uniform in (-1, 1], phi = 2 pi u4), |P| from the energy condition
-      // H = E: |P|^2 = 2 (E - eps H_p(X)) > 0 always (E > 2|eps|), so no point is off the shell (R28).
-      const double u1 = uniform01(seed, (uint64_t)K, 3), u2 = uniform01(seed, (uint64_t)K, 4);
-      const double ct = 1.0 - 2.0 * u1;
-      const double sth = std::sqrt((1.0 - ct) * (1.0 + ct));
-      const double ang = TWO_PI_HI * u2;
-      const double pn = std::sqrt(2.0 * (E - eps * Hp(X[0], X[1], X[2])));
-      status[k] = 1;
-      st[0] = X[0]; st[1] = X[1]; st[2] = X[2];
-      st[3] = pn * (sth * std::cos(ang));
-      st[4] = pn * (sth * std::sin(ang));
-      st[5] = (g->pz_sign < 0 ? -1.0 : 1.0) * (pn * ct);
-    } else {
-      double px, py;
-      if (g->shape == 0) {
-        px = g->lo_x + ((double)i + 0.5) * (g->hi_x - g->lo_x) / (double)g->gx;
-        py = g->lo_y + ((double)j + 0.5) * (g->hi_y - g->lo_y) / (double)g->gy;
-      } else {
-        const double u1 = uniform01(seed, (uint64_t)K, 3), u2 = uniform01(seed, (uint64_t)K, 4);
+    // P:97 "the corresponding initial velocity v_z was calculated from the fixed energy condition": a draw of
+    // (v_x, v_y, X) with 2(E - eps H_p(X)) < v_x^2 + v_y^2 has no real v_z.  Reading R31: with resample > 0 the
+    // trajectory is drawn again — attempt a takes ALL its draws (angles and cloud point) from the seed
+    // seed_a = seed + a * 0xD1B54A32D192ED03 (mod 2^64) — until it lies on the shell; the accepted points are
+    // distributed exactly like the unmasked points of the plain ensemble (rejection sampling).
+    const int attempts = (g->shape == 1 || g->shape == 2) && g->resample > 0 ? g->resample + 1 : 1;
+    for (int a = 0; a < attempts; ++a) {
+      const uint64_t sd = seed + (uint64_t)a * 0xD1B54A32D192ED03ull;
+      double X[3] = {0.0, 0.0, 0.0};
+      if (g->angle_mode == 1)
+        for (int al = 0; al < 3; ++al) X[al] = TWO_PI_HI * uniform01(sd, (uint64_t)K, (uint64_t)al);
+      if (g->shape == 3) {
+        // P:85 "initial conditions uniformly distributed over the sphere S": direction uniform on the unit
+        // sphere (cos(theta) = 1 - 2 u3 uniform in (-1, 1], phi = 2 pi u4), |P| from the energy condition
+        // H = E: |P|^2 = 2 (E - eps H_p(X)) > 0 always (E > 2|eps|), so no point is off the shell (R28).
+        const double u1 = uniform01(sd, (uint64_t)K, 3), u2 = uniform01(sd, (uint64_t)K, 4);
+        const double ct = 1.0 - 2.0 * u1;
+        const double sth = std::sqrt((1.0 - ct) * (1.0 + ct));
         const double ang = TWO_PI_HI * u2;
-        const double rad = (g->shape == 1) ? g->r * std::sqrt(u1)
-                                           : g->r * std::sqrt(-2.0 * std::log(1.0 - u1));
-        px = g->cx + rad * std::cos(ang);
-        py = g->cy + rad * std::sin(ang);
-      }
-      // third action from the energy condition H = E
-      double R = 2.0 * (E - eps * Hp(X[0], X[1], X[2]));
-      R = R - px * px;
-      R = R - py * py;
-      if (R < 0.0 || !(R == R)) {
-        status[k] = 0;
-        for (int c = 0; c < 6; ++c) st[c] = nan;
-      } else {
+        const double pn = std::sqrt(2.0 * (E - eps * Hp(X[0], X[1], X[2])));
         status[k] = 1;
         st[0] = X[0]; st[1] = X[1]; st[2] = X[2];
-        st[3] = px; st[4] = py;
-        st[5] = (g->pz_sign < 0 ? -1.0 : 1.0) * std::sqrt(R);
+        st[3] = pn * (sth * std::cos(ang));
+        st[4] = pn * (sth * std::sin(ang));
+        st[5] = (g->pz_sign < 0 ? -1.0 : 1.0) * (pn * ct);
+      } else {
+        double px, py;
+        if (g->shape == 0) {
+          px = g->lo_x + ((double)i + 0.5) * (g->hi_x - g->lo_x) / (double)g->gx;
+          py = g->lo_y + ((double)j + 0.5) * (g->hi_y - g->lo_y) / (double)g->gy;
+        } else {
+          const double u1 = uniform01(sd, (uint64_t)K, 3), u2 = uniform01(sd, (uint64_t)K, 4);
+          const double ang = TWO_PI_HI * u2;
+          const double rad = (g->shape == 1) ? g->r * std::sqrt(u1)
+                                             : g->r * std::sqrt(-2.0 * std::log(1.0 - u1));
+          px = g->cx + rad * std::cos(ang);
+          py = g->cy + rad * std::sin(ang);
+        }
+        // third action from the energy condition H = E
+        double R = 2.0 * (E - eps * Hp(X[0], X[1], X[2]));
+        R = R - px * px;
+        R = R - py * py;
+        if (R < 0.0 || !(R == R)) {
+          status[k] = 0;
+          for (int c = 0; c < 6; ++c) st[c] = nan;
+        } else {
+          status[k] = 1;
+          st[0] = X[0]; st[1] = X[1]; st[2] = X[2];
+          st[3] = px; st[4] = py;
+          st[5] = (g->pz_sign < 0 ? -1.0 : 1.0) * std::sqrt(R);
+        }
       }
+      if (status[k] == 1) break;
     }
     for (int c = 0; c < 6; ++c) q[c * pitch + k] = st[c];
     acc[0 * pitch + k] = 0.0;                                          // logsum

@@ -601,3 +601,44 @@ def test_gaussian_cloud_is_a_2d_normal(orc):
     assert abs(np.corrcoef(dx, dy)[0, 1]) < 0.012 and abs(dx.mean()) < 1.2e-4 and abs(dy.mean()) < 1.2e-4
     H = 0.5 * (s2.q[3:, :n] ** 2).sum(0) + np.cos(s2.q[0, :n]) * np.cos(s2.q[1, :n]) * (1 + np.cos(2 * s2.q[2, :n]))
     assert np.max(np.abs(H - 15.0)) < 64 * np.spacing(15.0)                 # v_z from the energy condition
+
+
+def test_cloud_resampling_is_rejection_sampling(orc):
+    """R31 (v_z "calculated from the fixed energy condition"; a draw without a real v_z is drawn again):
+    attempt a takes every draw of the trajectory from seed + a * 0xD1B54A32D192ED03.  Pinned by re-deriving the
+    accepted attempt from plain (resample = 0) ensembles generated with those seeds, and by the statistics: the
+    accepted points are distributed like the on-shell points of the plain ensemble (same conditional law)."""
+    n = 1 << 13
+    W = math.sqrt(15.0)
+    mk = lambda resample: orc.make_grid(128, 64, angle_mode=1, shape=2, cx=W, cy=W, r=0.01, resample=resample)
+    plain = [orc.init_shell(orc.State(n, tangent=False), mk(0), 15.0, 1.0, (7 + a * 0xD1B54A32D192ED03) % 2 ** 64)
+             for a in range(6)]
+    res = orc.init_shell(orc.State(n, tangent=False), mk(5), 15.0, 1.0, 7)
+    first = np.full(n, -1)
+    for a in reversed(range(6)):
+        first[plain[a].status == 1] = a
+    assert 0.3 < (first == 0).mean() < 0.7 and (first == 1).sum() > 0 and (first == 5).sum() > 0
+    assert np.array_equal(res.status == 1, first >= 0)
+    for a in range(6):
+        sel = first == a
+        assert np.array_equal(res.q[:, :n][:, sel], plain[a].q[:, :n][:, sel])
+        assert np.array_equal(res.acc[2, :n][sel], plain[a].acc[2, :n][sel])
+    assert np.isnan(res.q[:, :n][:, first < 0]).all()
+    # enough attempts: everyone is on the shell (P(all 40 draws fail) ~ 2^-40), H = E for all
+    full = orc.init_shell(orc.State(n, tangent=False), mk(40), 15.0, 1.0, 7)
+    assert np.all(full.status == 1) and np.max(np.abs(full.acc[2, :n] - 15.0)) < 64 * np.spacing(15.0)
+    # same conditional law as the masked ensemble: compare the first two moments of (px, py) and of H_p
+    big = orc.init_shell(orc.State(1 << 16, tangent=False), orc.make_grid(256, 256, angle_mode=1, shape=2, cx=W, cy=W,
+                                                                         r=0.01), 15.0, 1.0, 99)
+    lv = big.status == 1
+    hp = lambda s, m: (np.cos(s.q[0, :s.n]) * np.cos(s.q[1, :s.n]) * (1 + np.cos(2 * s.q[2, :s.n])))[m]
+    all_live = np.ones(n, bool)
+    assert abs(hp(full, all_live).mean() - hp(big, lv).mean()) < 0.03           # both ~ E[H_p | on shell] < 0
+    assert hp(full, all_live).max() < 0.3 and hp(big, lv).mean() < -0.3      # 2 H_p <= 2E - px^2 - py^2 ~ +-0.1
+    assert abs(full.q[3, :n].mean() - big.q[3, :big.n][lv].mean()) < 5e-4
+    assert abs(full.q[3, :n].std() - big.q[3, :big.n][lv].std()) < 5e-4
+    # grids and the sphere ignore the flag
+    for shape in (0, 3):
+        a_ = orc.init_shell(orc.State(64, tangent=False), orc.make_grid(8, 8, angle_mode=1, shape=shape, resample=0), 1.0, 3e-2, 1)
+        b_ = orc.init_shell(orc.State(64, tangent=False), orc.make_grid(8, 8, angle_mode=1, shape=shape, resample=9), 1.0, 3e-2, 1)
+        assert np.array_equal(a_.q, b_.q, equal_nan=True)
