@@ -162,7 +162,7 @@ def oracle_rate(cfg, order, tangent, seconds, cores=None):
     st = oracle.State(sub * sub, tangent=tangent, wind=True)
     st.order = order
     g = oracle.make_grid(sub, sub, cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"], cfg["cx"],
-                         cfg["cy"], cfg["r"])
+                         cfg["cy"], cfg["r"], resample=cfg.get("resample", 0))
     oracle.init_shell(st, g, cfg["E"], cfg["eps"], cfg["seed"])
     live = int((st.status == 1).sum())
 
@@ -195,7 +195,7 @@ def oracle_live_count(cfg, world, scaling):
     gx, gy_total, _, _ = parallel.slice_of(cfg["gx"], cfg["gy"], world, 0, scaling)
     st = oracle.State(gx * gy_total, tangent=False, wind=False)
     g = oracle.make_grid(gx, gy_total, cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"], cfg["cx"], cfg["cy"],
-                         cfg["r"])
+                         cfg["r"], resample=cfg.get("resample", 0))
     oracle.init_shell(st, g, cfg["E"], cfg["eps"], cfg["seed"])
     return int((st.status == 1).sum())
 
@@ -280,7 +280,7 @@ def run_ours(args, cfg, order, tangent):
     counts = [parallel.slice_of(cfg["gx"], cfg["gy"], world, r, args.scaling)[3] for r in range(world)]
     horizon = effective_horizon(args, cfg)
     grid = aw.make_grid(gx, gy_total, cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"], cfg["cx"], cfg["cy"],
-                        cfg["r"], 1, 0, k0=k0)
+                        cfg["r"], 1, 0, k0=k0, resample=cfg.get("resample", 0))
     dens_mode = cfg.get("density_mode", 0)          # 0: instantaneous actions; 1-3: the paper's averaged velocity
     window = cfg.get("window", 0)                   # > 0: consecutive averaging windows, density accumulated (Fig. 4)
     every = cfg.get("density_every", 0)             # > 0: instantaneous density binned every `every` steps (configs[4])

@@ -128,6 +128,14 @@ typedef struct {
                                    position and every random draw are functions of the GLOBAL index K, so a slice
                                    is bit-identical to the same rows of the whole (multi-GPU sharding, P:13, P:63;
                                    R30): rank r of a row-sharded job passes k0 = j0*gx, n = rows*gx          */
+  int32_t resample;             /* shapes DISK, GAUSS: a draw (px, py, X) with 2(E - eps H_p(X)) < px^2 + py^2 has no
+                                   real third action ("v_z from the fixed energy condition").  0: mask it (status
+                                   0, R8).  m > 0: draw the trajectory again, up to m times — attempt a takes ALL its
+                                   draws (angles, cloud point) from seed_a = seed + a*0xD1B54A32D192ED03 (mod 2^64) —
+                                   until it is on the shell (rejection sampling: the accepted points are distributed
+                                   like the unmasked points of the plain ensemble; R31).  Every trajectory is then
+                                   live (up to probability P(off shell)^(m+1)), so no warp lane idles            */
+  int32_t reserved_;
 } aw_grid;
 
 /* Bytes the caller must provide for each buffer.  *pitch_out = n rounded up to a multiple of 32.

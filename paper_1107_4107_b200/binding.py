@@ -47,7 +47,8 @@ class Grid(C.Structure):
                 ("lo_x", C.c_double), ("hi_x", C.c_double), ("lo_y", C.c_double), ("hi_y", C.c_double),
                 ("angle_mode", C.c_int32), ("shape", C.c_int32),
                 ("cx", C.c_double), ("cy", C.c_double), ("r", C.c_double),
-                ("pz_sign", C.c_int32), ("tangent_mode", C.c_int32), ("k0", C.c_int64)]
+                ("pz_sign", C.c_int32), ("tangent_mode", C.c_int32), ("k0", C.c_int64),
+                ("resample", C.c_int32), ("reserved_", C.c_int32)]
 
 
 class HostIn(C.Structure):
@@ -61,11 +62,11 @@ class HostOut(C.Structure):
 
 
 def make_grid(gx, gy, lo=-1.0, hi=1.0, angle_mode=0, shape=0, cx=0.0, cy=0.0, r=0.0, pz_sign=1,
-              tangent_mode=0, lo_y=None, hi_y=None, k0=0):
+              tangent_mode=0, lo_y=None, hi_y=None, k0=0, resample=0):
     """The grid describes the WHOLE ensemble of gx*gy trajectories; an Ensemble of n trajectories initialised with
     it holds the slice [k0, k0 + n) (include/aw.h, aw_grid.k0)."""
     return Grid(gx, gy, lo, hi, lo if lo_y is None else lo_y, hi if hi_y is None else hi_y,
-                angle_mode, shape, cx, cy, r, pz_sign, tangent_mode, k0)
+                angle_mode, shape, cx, cy, r, pz_sign, tangent_mode, k0, resample, 0)
 
 
 _lib = None

@@ -33,47 +33,51 @@ __global__ void __launch_bounds__(256) init_shell_kernel(const __grid_constant__
   const int64_t i = K % g.gx, j = K / g.gx;
   const uint64_t uk = (uint64_t)K;
 
-  double x = 0.0, y = 0.0, z = 0.0;
-  if (g.angle_mode == 1) {
-    x = kTwoPiHi * uniform01(p.seed, uk, 0);
-    y = kTwoPiHi * uniform01(p.seed, uk, 1);
-    z = kTwoPiHi * uniform01(p.seed, uk, 2);
-  }
   const double nan = __longlong_as_double(0x7ff8000000000000ll);
   const double sgn = g.pz_sign < 0 ? -1.0 : 1.0;
-  double px, py, pz = nan, H0 = nan;
-  bool live;
-  if (g.shape == AW_SHAPE_SPHERE) {
-    // direction uniform on the unit sphere, |P| from the energy condition (R28); always on the shell
-    const double u1 = uniform01(p.seed, uk, 3), u2 = uniform01(p.seed, uk, 4);
-    const double ct = __dsub_rn(1.0, __dmul_rn(2.0, u1));
-    const double sth = sqrt(__dmul_rn(__dsub_rn(1.0, ct), __dadd_rn(1.0, ct)));
-    double sn, cs;
-    sincos(kTwoPiHi * u2, sn, cs);
-    const double pn = sqrt(__dmul_rn(2.0, __dsub_rn(p.E, __dmul_rn(p.eps, hp_dev(x, y, z)))));
-    px = __dmul_rn(pn, __dmul_rn(sth, cs));
-    py = __dmul_rn(pn, __dmul_rn(sth, sn));
-    pz = sgn * __dmul_rn(pn, ct);
-    live = true;
-  } else {
-    if (g.shape == AW_SHAPE_GRID) {
-      px = __dadd_rn(g.lo_x, __ddiv_rn(__dmul_rn(__dadd_rn((double)i, 0.5), __dsub_rn(g.hi_x, g.lo_x)), (double)g.gx));
-      py = __dadd_rn(g.lo_y, __ddiv_rn(__dmul_rn(__dadd_rn((double)j, 0.5), __dsub_rn(g.hi_y, g.lo_y)), (double)g.gy));
-    } else {
-      const double u1 = uniform01(p.seed, uk, 3), u2 = uniform01(p.seed, uk, 4);
-      const double rad = (g.shape == AW_SHAPE_DISK) ? __dmul_rn(g.r, sqrt(u1))
-                                                    : __dmul_rn(g.r, sqrt(-2.0 * log(1.0 - u1)));
+  double x = 0.0, y = 0.0, z = 0.0, px = nan, py = nan, pz = nan, H0 = nan;
+  bool live = false;
+  // cloud shapes with resample > 0: draw again until the point has a real third action (R31; include/aw.h)
+  const int attempts = (g.shape == AW_SHAPE_DISK || g.shape == AW_SHAPE_GAUSS) && g.resample > 0 ? g.resample + 1 : 1;
+  for (int a = 0; a < attempts && !live; ++a) {
+    const uint64_t sd = p.seed + (uint64_t)a * 0xD1B54A32D192ED03ull;
+    if (g.angle_mode == 1) {
+      x = kTwoPiHi * uniform01(sd, uk, 0);
+      y = kTwoPiHi * uniform01(sd, uk, 1);
+      z = kTwoPiHi * uniform01(sd, uk, 2);
+    }
+    if (g.shape == AW_SHAPE_SPHERE) {
+      // direction uniform on the unit sphere, |P| from the energy condition (R28); always on the shell
+      const double u1 = uniform01(sd, uk, 3), u2 = uniform01(sd, uk, 4);
+      const double ct = __dsub_rn(1.0, __dmul_rn(2.0, u1));
+      const double sth = sqrt(__dmul_rn(__dsub_rn(1.0, ct), __dadd_rn(1.0, ct)));
       double sn, cs;
       sincos(kTwoPiHi * u2, sn, cs);
-      px = __dadd_rn(g.cx, __dmul_rn(rad, cs));
-      py = __dadd_rn(g.cy, __dmul_rn(rad, sn));
+      const double pn = sqrt(__dmul_rn(2.0, __dsub_rn(p.E, __dmul_rn(p.eps, hp_dev(x, y, z)))));
+      px = __dmul_rn(pn, __dmul_rn(sth, cs));
+      py = __dmul_rn(pn, __dmul_rn(sth, sn));
+      pz = sgn * __dmul_rn(pn, ct);
+      live = true;
+    } else {
+      if (g.shape == AW_SHAPE_GRID) {
+        px = __dadd_rn(g.lo_x, __ddiv_rn(__dmul_rn(__dadd_rn((double)i, 0.5), __dsub_rn(g.hi_x, g.lo_x)), (double)g.gx));
+        py = __dadd_rn(g.lo_y, __ddiv_rn(__dmul_rn(__dadd_rn((double)j, 0.5), __dsub_rn(g.hi_y, g.lo_y)), (double)g.gy));
+      } else {
+        const double u1 = uniform01(sd, uk, 3), u2 = uniform01(sd, uk, 4);
+        const double rad = (g.shape == AW_SHAPE_DISK) ? __dmul_rn(g.r, sqrt(u1))
+                                                      : __dmul_rn(g.r, sqrt(-2.0 * log(1.0 - u1)));
+        double sn, cs;
+        sincos(kTwoPiHi * u2, sn, cs);
+        px = __dadd_rn(g.cx, __dmul_rn(rad, cs));
+        py = __dadd_rn(g.cy, __dmul_rn(rad, sn));
+      }
+      // third action from the energy condition H = E: pz^2 = 2(E - eps H_p) - px^2 - py^2
+      double R = __dmul_rn(2.0, __dsub_rn(p.E, __dmul_rn(p.eps, hp_dev(x, y, z))));
+      R = __dsub_rn(R, __dmul_rn(px, px));
+      R = __dsub_rn(R, __dmul_rn(py, py));
+      live = R >= 0.0;  // false for NaN too
+      if (live) pz = sgn * sqrt(R);
     }
-    // third action from the energy condition H = E: pz^2 = 2(E - eps H_p) - px^2 - py^2
-    double R = __dmul_rn(2.0, __dsub_rn(p.E, __dmul_rn(p.eps, hp_dev(x, y, z))));
-    R = __dsub_rn(R, __dmul_rn(px, px));
-    R = __dsub_rn(R, __dmul_rn(py, py));
-    live = R >= 0.0;  // false for NaN too
-    if (live) pz = sgn * sqrt(R);
   }
   if (live) {
     H0 = hamiltonian_dev(x, y, z, px, py, pz, p.eps);

@@ -74,10 +74,39 @@ def test_gauss_init_matches_oracle_generator(aw, orc, E, eps, cx, cy, sigma, pz_
         assert np.allclose(got.w[:, :n], ref.w[:, :n], rtol=0, atol=2e-15)
 
 
+@pytest.mark.parametrize("shape,resample", [(2, 3), (2, 40), (1, 5)])
+def test_cloud_resampling_matches_oracle_generator(aw, orc, shape, resample):
+    """R31: draws without a real v_z are drawn again from the attempt seeds; the device generator accepts the same
+    attempt as the oracle's for every trajectory (up to a radicand at the rounding level), k0 slices included."""
+    W = math.sqrt(15.0)
+    gx, gy, k0 = 97, 61, 1000
+    n = gx * gy - k0 - 7
+    mk = lambda mod: mod.make_grid(gx, gy, angle_mode=1, shape=shape, cx=W, cy=W, r=0.01 if shape == 2 else 0.02,
+                                   k0=k0, resample=resample)
+    ens = aw.Ensemble(n, tangent=False, wind=True)
+    aw.aw_init_shell(ens, mk(aw), 15.0, 1.0, 31)
+    ref = orc.init_shell(orc.State(n, tangent=False), mk(orc), 15.0, 1.0, 31)
+    got = ensemble_to_oracle(ens, orc)
+    both = (got.status == 1) & (ref.status == 1)
+    same = both & np.all(got.q[:3, :n] == ref.q[:3, :n], axis=0)
+    assert (got.status != ref.status).sum() + (both & ~same).sum() <= 2
+    if resample == 40:
+        assert np.all(ref.status == 1) and np.all(got.status == 1)
+    else:
+        assert 0 < (ref.status == 0).sum() < 0.2 * n              # P(off shell)^(resample + 1) of the draws remain masked
+    assert np.max(np.abs(got.q[3:5, :n][:, same] - ref.q[3:5, :n][:, same])) <= 4e-14
+    assert np.max(np.abs(got.q[5, :n][same] ** 2 - ref.q[5, :n][same] ** 2)) <= 64 * ULP1 * 34.0
+    assert np.max(np.abs(got.acc[2, :n][got.status == 1] - 15.0)) <= 16 * np.spacing(15.0)
+    bad = mk(aw)
+    bad.resample = -1
+    with pytest.raises(aw.AwError):
+        aw.aw_init_shell(ens, bad, 15.0, 1.0, 31)
+
+
 # ------------------------------------------------------------------ P:97 Fig. 4: consecutive windows
 
 def test_fig4_consecutive_windows_density_parity(aw, orc):
-    """CONFIGS[7] (N = 3.2e4 live trajectories in a Gaussian cloud at W, E = 15, eps = 1, order 6, h = 0.01 T) in the
+    """CONFIGS[7] (N = 3.2e4 trajectories in a Gaussian cloud at W, resampled onto the shell, E = 15, eps = 1, order 6, h = 0.01 T) in the
     launch configuration bench.py --config 7 times: windows x (aw_mark; aw_integrate(Dt = 50 T); aw_density mode 3
     ACCUMULATING) = the density "averaged over the whole time span between consecutive plots".  After each of
     three consecutive windows the accumulated histogram is bit-exact against the oracle's binning of the device
@@ -86,12 +115,20 @@ def test_fig4_consecutive_windows_density_parity(aw, orc):
     n = cfg["gx"] * cfg["gy"]
     ens = aw.Ensemble(n, tangent=False, wind=True, order=cfg["order"], ref=True)
     g = aw.make_grid(cfg["gx"], cfg["gy"], cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"], cfg["cx"], cfg["cy"],
-                     cfg["r"])
+                     cfg["r"], resample=cfg["resample"])
     aw.aw_init_shell(ens, g, cfg["E"], cfg["eps"], cfg["seed"])
     assert aw.aw_trig_level(ens, cfg["dt"]) == 7
     st0 = ensemble_to_oracle(ens, orc)
     live0 = st0.status == 1
-    assert 30_000 < live0.sum() < 34_000                        # the paper's N = 3.2e4
+    assert n == 32_000 and live0.all()                          # the paper's N = 3.2e4, every draw on the shell
+    # the generator with resampling (R31) against the oracle's: same accepted attempt for every trajectory
+    gen = orc.init_shell(orc.State(n, tangent=False), orc.make_grid(cfg["gx"], cfg["gy"], cfg["lo"], cfg["hi"],
+                         cfg["angle_mode"], cfg["shape"], cfg["cx"], cfg["cy"], cfg["r"], resample=cfg["resample"]),
+                         cfg["E"], cfg["eps"], cfg["seed"])
+    assert np.all(gen.status == 1)
+    same = np.all(gen.q[:3, :n] == st0.q[:3, :n], axis=0)        # angles are hash * constant: equal iff same attempt
+    assert (~same).sum() <= 2                                    # radicand at the rounding level may flip an attempt
+    assert np.max(np.abs(gen.q[3:5, :n][:, same] - st0.q[3:5, :n][:, same])) <= 4e-14
     # state parity, 100 steps, on 512 sampled live trajectories (the region around W is strongly chaotic)
     sample = np.nonzero(live0)[0][:: max(1, int(live0.sum()) // 512)][:512]
     probe = aw.Ensemble(n, tangent=False, wind=True, order=cfg["order"])
