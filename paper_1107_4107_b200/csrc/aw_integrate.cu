@@ -17,7 +17,7 @@
 //   grad H_p = -(F sin u, F sin v, (cos u + cos v) sin zeta),  F = 1 + cos zeta   (d/du, d/dv, d/dz),
 // and the Hessian-vector product is the sum and difference of the x and y rows of SURVEY.md Appendix A.2.
 //
-// Trigonometry.  LEVEL 0: the device sincos (aw_trig.cuh) of u, v, zeta at every stage.
+// Trigonometry.  LEVEL 0: the table-driven sincos (tsincos below) of u, v, zeta at every stage.
 // LEVEL >= 1: the pairs (sin u, cos u), (sin v, cos v), (sin zeta, cos zeta) are carried in registers and
 // advanced through every drift by the rotation with the drift angle d = a p (p = pu, pv, pzeta):
 //     s' = s + (s m + c g),  c' = c + (c m - s g),   g = sin d = p G(p^2),  m = cos d - 1 = p^2 M(p^2),
@@ -39,6 +39,7 @@
 #include "aw_internal.cuh"
 #include "aw_model.cuh"
 #include "aw_trig.cuh"
+#include "aw_trig_table.h"
 
 #ifndef AW_BLOCK
 #define AW_BLOCK 128
@@ -100,6 +101,41 @@ __device__ __forceinline__ void rotate(double &s, double &c, double g, double m)
   c = c1;
 }
 
+// Table-driven sincos for the kicks that follow a drift too long to rotate through (levels 0 and 6-9): the angle is
+// split as x = k (2 pi / T) + r, |r| <= pi / T, the pair of the grid point k mod T comes from a table of T correctly
+// rounded (sin, cos) values in shared memory (csrc/aw_trig_table.h, whole circle), and is rotated by the residual
+// r with the same short Taylor series as the drift rotations (T = 1024: degree 2, truncation r^6/720 < 1.2e-18).
+// Against the device sincos of aw_trig.cuh (19 fp64 + ~12 integer-pipe instructions for the quadrant swap and signs)
+// this is 14 fp64 + 3 (index mask, address, 16-byte shared load): there is no quadrant logic, and it was the integer
+// work, one issue cycle each, that held the sincos-bound kernels at ~80 % of the fp64 pipe (profiles/r2a_*).
+// Exact at x = 0 (r = 0, entry 0 = (0, 1)); the table is mirror-symmetric, so sin stays bit-odd and cos bit-even.
+constexpr int kTab = 1 << AW_TAB_LOG2;
+
+__device__ __forceinline__ void tsincos(const double2 *__restrict__ tab, double x, double &s, double &c) {
+  const double j = fma(x, AW_TAB_INV_STEP, kRintMagic);  // round-to-nearest-even of x T / 2 pi in the low mantissa bits
+  const int q = __double2loint(j);
+  const double k = j - kRintMagic;
+  double r = fma(-k, AW_TAB_STEP_HI, x);                 // exact: the difference is representable (|x| < 1024, R7)
+  r = fma(-k, AW_TAB_STEP_LO, r);
+  const double2 e = tab[q & (kTab - 1)];
+  const double z = r * r;
+  double pg, pm;
+  if (AW_TAB_LOG2 >= 10) {                               // |r| <= 0.00307
+    pg = fma(z, 0x1.1111111111111p-7, -0x1.5555555555555p-3);    //  1/120, -1/6
+    pm = fma(z, 0x1.5555555555555p-5, -0.5);                     //  1/24
+  } else {                                               // T = 256: |r| <= 0.0123, one more term
+    pg = fma(z, -0x1.a01a01a01a01ap-13, 0x1.1111111111111p-7);   // -1/5040
+    pg = fma(pg, z, -0x1.5555555555555p-3);
+    pm = fma(z, -0x1.6c16c16c16c17p-10, 0x1.5555555555555p-5);   // -1/720
+    pm = fma(pm, z, -0.5);
+  }
+  const double g = fma(r * z, pg, r);                    // sin r
+  const double m = z * pm;                               // cos r - 1
+  const double t1 = fma(e.x, m, e.x), t2 = fma(e.y, m, e.y);
+  s = fma(e.y, g, t1);
+  c = fma(-e.x, g, t2);
+}
+
 // Taylor degrees of the drift rotations.  A trigonometry level L is picked on the host from
 // |d| = max_s |a_s| max|P| <= kLevelMaxD[L] (trig_level_for).  The drift after kick s has its own constant
 // a_loop[s]; its ratio to the largest one is fixed by the scheme (kDriftRatio, checked on the host), so each
@@ -122,20 +158,35 @@ template <int S> struct DriftRatio;
 template <> struct DriftRatio<3> { static constexpr double r[3] = {0.1300, 0.1300, 1.0}; };
 template <> struct DriftRatio<7> { static constexpr double r[7] = {0.6502, 0.6005, 0.08765, 0.08765, 0.6005, 0.6502, 1.0}; };
 
+// A degree-N rotation costs 2N + 6 fp64 instructions per pair, the table-driven sincos 14 + 3 light ones: beyond
+// degree kMaxRotDegree the drift leaves the pairs stale and the kick that follows evaluates tsincos instead.
+#ifndef AW_MAX_ROT_DEGREE
+#define AW_MAX_ROT_DEGREE 5
+#endif
+constexpr int kMaxRotDegree = AW_MAX_ROT_DEGREE;
+
 template <int S, int LEVEL, int cs, bool ZETA>
 __host__ __device__ constexpr int rotation_degree() {
-  if (LEVEL == 0) return 0;  // no rotation: device sincos at every stage
+  if (LEVEL == 0) return 0;  // no rotation: table-driven sincos at every stage
   const double t = (ZETA ? 2.0 : 1.4142135623730951) * kLevelMaxD[LEVEL] * DriftRatio<S>::r[cs];
   int n = 1;
-  while (n < 8 && kDegreeMaxAngle[n] < t) ++n;
-  return kDegreeMaxAngle[n] < t ? 0 : n;  // 0: the angle is too large for a degree-8 rotation
+  while (n < kMaxRotDegree && kDegreeMaxAngle[n] < t) ++n;
+  return kDegreeMaxAngle[n] < t ? 0 : n;  // 0: the angle is too large for a rotation of degree <= kMaxRotDegree
 }
 
-// does the drift after kick s rotate the running pairs (true at levels 1-7, per drift at level 8, never at 0)?
+// does the drift after kick s rotate the running pairs (true at levels 1-5, per drift at levels 6-9, never at 0)?
 template <int S, int LEVEL, int s>
 __host__ __device__ constexpr bool drift_rotates() {
   constexpr int cs = (s == S - 1) ? s : (s < S - 2 - s ? s : S - 2 - s);
   return rotation_degree<S, LEVEL, cs, false>() > 0 && rotation_degree<S, LEVEL, cs, true>() > 0;
+}
+// Do all drifts of a step rotate?  Then the pairs live on rotations alone and are re-synchronised from the angles
+// every chunk; otherwise every step contains a kick that recomputes them from the angles (tsincos) and the kernel
+// needs the table.
+template <int S, int LEVEL, int s = 0>
+__host__ __device__ constexpr bool all_drifts_rotate() {
+  if constexpr (s == S) return true;
+  else return drift_rotates<S, LEVEL, s>() && all_drifts_rotate<S, LEVEL, s + 1>();
 }
 
 // Everything a thread carries between stages.  Inside a block of `stride` steps the state is held in the
@@ -218,9 +269,9 @@ __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
   }
 }
 
-template <bool TAN, int LEVEL>
+template <int S, bool TAN, int LEVEL>
 __device__ __forceinline__ void resync(Traj<TAN> &t) {
-  if (LEVEL > 0 && LEVEL < 8) {  // levels 8, 9 recompute the pairs with the device sincos in every step
+  if constexpr (all_drifts_rotate<S, LEVEL>()) {  // otherwise a kick of every step recomputes the pairs anyway
     sincos(t.u, t.su, t.cu);
     sincos(t.v, t.sv, t.cv);
     sincos(t.zt, t.s2, t.c2);
@@ -236,11 +287,11 @@ __device__ __forceinline__ void resync(Traj<TAN> &t) {
 // (the sum and difference of the x and y rows of SURVEY.md Appendix A.2, with dzeta = 2 dz).
 // FRESH: the running pairs are valid (the drift before this kick rotated them); otherwise they are evaluated here.
 template <bool TAN, bool FRESH>
-__device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2) {
+__device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2, const double2 *__restrict__ tab) {
   if (!FRESH) {
-    sincos(t.u, t.su, t.cu);
-    sincos(t.v, t.sv, t.cv);
-    sincos(t.zt, t.s2, t.c2);
+    tsincos(tab, t.u, t.su, t.cu);
+    tsincos(tab, t.v, t.sv, t.cv);
+    tsincos(tab, t.zt, t.s2, t.c2);
   }
   const double F = fma(b1, t.c2, b1);  // b (1 + cos zeta)
   const double G2 = b2 * t.s2;         // 2 b sin zeta
@@ -260,18 +311,27 @@ __device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2) {
 
 // stages s, s+1, ..., S-1 of one step: kick_s then the drift after it
 template <int S, bool TAN, int LEVEL, int s>
-__device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p) {
+__device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p, const double2 *__restrict__ tab) {
   if constexpr (s < S) {
     // the drift before kick s is the one after kick s-1, or for s = 0 the merged drift that closed the last step
-    kick<TAN, drift_rotates<S, LEVEL, (s == 0 ? S - 1 : s - 1)>()>(t, p.b1[s], p.b2[s]);
+    kick<TAN, drift_rotates<S, LEVEL, (s == 0 ? S - 1 : s - 1)>()>(t, p.b1[s], p.b2[s], tab);
     drift<S, TAN, LEVEL, s>(t, p);
-    stages<S, TAN, LEVEL, s + 1>(t, p);
+    stages<S, TAN, LEVEL, s + 1>(t, p, tab);
   }
 }
 
 template <int S, bool TAN, int LEVEL>
 __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS(LEVEL))
     integrate_kernel(const __grid_constant__ IntegrateParams p) {
+  // the (sin, cos) table of tsincos, whole circle, 16 KB of shared memory per block (kernels with a stale drift only)
+  constexpr bool kUsesTable = !all_drifts_rotate<S, LEVEL>();
+  __shared__ double2 tab_s[kUsesTable ? kTab : 1];
+  if constexpr (kUsesTable) {
+    for (int i = threadIdx.x; i < kTab; i += blockDim.x)
+      tab_s[i] = make_double2(aw_trig_table[2 * i], aw_trig_table[2 * i + 1]);
+    __syncthreads();
+  }
+  const double2 *tab = tab_s;
   // blocks of 32, 64 or 128 threads (launch_one): the arithmetic is per trajectory, so the result does not depend on it
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= p.n) return;
@@ -292,15 +352,15 @@ __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS(LEVEL))
     const double px0 = t.pu, py0 = t.pv;
     rotate_in<TAN>(t);                              // (x, y, z) -> (u, v, zeta)
     drift_angles<TAN>(t, p.a_open, 2.0 * p.a_open);  // opening drift of the block
-    resync<TAN, LEVEL>(t);           // pairs from the angles: the same values a new launch would start from
+    resync<S, TAN, LEVEL>(t);        // pairs from the angles: the same values a new launch would start from
 
 #pragma unroll 1
     for (int rem = p.stride; rem > 0;) {
       const int m = rem < p.chunk ? rem : p.chunk;
       rem -= m;
 #pragma unroll 1
-      for (int i = m; i > 0; --i) stages<S, TAN, LEVEL, 0>(t, p);
-      if (rem > 0) resync<TAN, LEVEL>(t);
+      for (int i = m; i > 0; --i) stages<S, TAN, LEVEL, 0>(t, p, tab);
+      if (rem > 0) resync<S, TAN, LEVEL>(t);
     }
     drift_angles<TAN>(t, -p.a_open, -2.0 * p.a_open);  // last merged drift -> closing drift of the block
     rotate_out<TAN>(t, px0, py0);                      // (u, v, zeta) -> (x, y, z)
