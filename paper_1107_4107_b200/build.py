@@ -57,9 +57,10 @@ def build(force=False, verbose=False, extra_flags=()):
     build_dir = os.path.join(HERE, "build")
     os.makedirs(build_dir, exist_ok=True)
     log = []
+    extra_flags = list(extra_flags) + os.environ.get("AW_EXTRA_NVCC_FLAGS", "").split()   # tuning experiments only
     for src, objname, unit_flags in UNITS:
         obj = os.path.join(build_dir, objname)
-        cmd = [_nvcc()] + NVCC_FLAGS + unit_flags + list(extra_flags) + ["-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [_nvcc()] + NVCC_FLAGS + unit_flags + extra_flags + ["-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         log.append(r.stderr)
         if r.returncode != 0:

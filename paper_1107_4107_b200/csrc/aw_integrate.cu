@@ -101,35 +101,45 @@ __device__ __forceinline__ void rotate(double &s, double &c, double g, double m)
   c = c1;
 }
 
-// Table-driven sincos for the kicks that follow a drift too long to rotate through (levels 0 and 6-9): the angle is
-// split as x = k (2 pi / T) + r, |r| <= pi / T, the pair of the grid point k mod T comes from a table of T correctly
-// rounded (sin, cos) values in shared memory (csrc/aw_trig_table.h, whole circle), and is rotated by the residual
-// r with the same short Taylor series as the drift rotations (T = 1024: degree 2, truncation r^6/720 < 1.2e-18).
+// Table-driven sincos for the kicks that follow a drift too long to rotate through (from level 4 on, and at every
+// stage of level 0): the angle is split as x = k (2 pi / T) + r, |r| <= pi / T, the pair of the grid point k mod T comes
+// from a table of T = 256 correctly rounded (sin, cos) values in shared memory (csrc/aw_trig_table.h, whole circle),
+// and is rotated by the residual r with the same short Taylor series as the drift rotations (|r| <= 0.0123: sin to
+// r^5, truncation 8e-18; cos - 1 to r^6, truncation 1e-20).
 // Against the device sincos of aw_trig.cuh (19 fp64 + ~12 integer-pipe instructions for the quadrant swap and signs)
-// this is 14 fp64 + 3 (index mask, address, 16-byte shared load): there is no quadrant logic, and it was the integer
+// this is 15 fp64 + 3 (shift, mask-or, 16-byte shared load): there is no quadrant logic, and it was the integer
 // work, one issue cycle each, that held the sincos-bound kernels at ~80 % of the fp64 pipe (profiles/r2a_*).
+// Shared-memory layout: the lanes of a warp look up unrelated entries, and a 16-byte load is served a quarter-warp
+// (8 lanes) at a time, so a plain array costs ~10 wavefronts per load in bank conflicts and the kernel becomes
+// shared-memory bound (profiles/r2b_*: l1tex data-pipe wavefronts 99.7 % of peak).  The table is therefore stored 8
+// times, row k = the 8 copies of entry k (128 bytes = all 32 banks), and lane l reads copy l mod 8: the 8 lanes of a
+// quarter-warp hit 8 different bank groups whatever their k, i.e. 4 wavefronts per load, the minimum.  32 KB per block.
 // Exact at x = 0 (r = 0, entry 0 = (0, 1)); the table is mirror-symmetric, so sin stays bit-odd and cos bit-even.
 constexpr int kTab = 1 << AW_TAB_LOG2;
+constexpr int kTabCopies = 4;
+static_assert(AW_TAB_LOG2 == 9, "tsincos: the polynomial degrees below are sized for T = 512");
 
-__device__ __forceinline__ void tsincos(const double2 *__restrict__ tab, double x, double &s, double &c) {
+// The table handle a thread carries: the shared array and the byte offset of its copy, (lane mod 8) * 16.  The entry
+// address is base + (((q << 7) & ((T - 1) << 7)) | lane_off): one shift, one three-input logic op, one load.
+struct TrigTable {
+  const char *base;
+  unsigned lane_off;
+};
+
+__device__ __forceinline__ void tsincos(const TrigTable &tab, double x, double &s, double &c) {
   const double j = fma(x, AW_TAB_INV_STEP, kRintMagic);  // round-to-nearest-even of x T / 2 pi in the low mantissa bits
   const int q = __double2loint(j);
   const double k = j - kRintMagic;
   double r = fma(-k, AW_TAB_STEP_HI, x);                 // exact: the difference is representable (|x| < 1024, R7)
   r = fma(-k, AW_TAB_STEP_LO, r);
-  const double2 e = tab[q & (kTab - 1)];
+  const unsigned off = (((unsigned)q << 6) & ((unsigned)(kTab - 1) << 6)) | tab.lane_off;
+  const double2 e = *reinterpret_cast<const double2 *>(tab.base + off);
   const double z = r * r;
-  double pg, pm;
-  if (AW_TAB_LOG2 >= 10) {                               // |r| <= 0.00307
-    pg = fma(z, 0x1.1111111111111p-7, -0x1.5555555555555p-3);    //  1/120, -1/6
-    pm = fma(z, 0x1.5555555555555p-5, -0.5);                     //  1/24
-  } else {                                               // T = 256: |r| <= 0.0123, one more term
-    pg = fma(z, -0x1.a01a01a01a01ap-13, 0x1.1111111111111p-7);   // -1/5040
-    pg = fma(pg, z, -0x1.5555555555555p-3);
-    pm = fma(z, -0x1.6c16c16c16c17p-10, 0x1.5555555555555p-5);   // -1/720
-    pm = fma(pm, z, -0.5);
-  }
-  const double g = fma(r * z, pg, r);                    // sin r
+  const double pg = fma(z, 0x1.1111111111111p-7, -0x1.5555555555555p-3);      //  1/120, -1/6
+  const double pm = fma(z, AW_TAB_COS_C1, -0.5);                             //  1/24 adjusted (economised), -1/2
+  // sin r = r (1 + z pg): the rounding of 1 + z pg (1 ulp of a correction below 0.013) is far below ulp(sin x), and
+  // the product form keeps every instruction at two register operands (a three-register DFMA issues in 3 cycles)
+  const double g = r * fma(z, pg, 1.0);
   const double m = z * pm;                               // cos r - 1
   const double t1 = fma(e.x, m, e.x), t2 = fma(e.y, m, e.y);
   s = fma(e.y, g, t1);
@@ -145,11 +155,11 @@ __device__ __forceinline__ void tsincos(const double2 *__restrict__ tab, double 
 //   N = 1: t <= 6.8e-5;  2: 0.00293;  3: 0.0208;  4: 0.0708;  5: 0.165;  6: 0.310;  7: 0.505;  8: 0.750.
 // The largest drift (the merged one) gets degrees (3,3), (3,4), (4,4), (4,5), (5,6), (6,7), (7,8) at levels
 // 1..7; the short inner drifts of the triple jump (ratio 0.13) and of the 7-stage scheme (0.088) one or two less.
-// Levels 8 (|d| <= 0.54) and 9 (|d| <= 2) are mixed: a drift whose own largest angle still fits degree <= 8 rotates
-// the pairs, the others leave them stale and the kick that follows evaluates the device sincos instead (degree 0
-// below).  Level 8: the inner drifts of the triple jump (two of three stages) and all six inner drifts of the
-// 7-stage scheme rotate; level 9: the triple jump's two, and the 7-stage scheme's two 0.088 drifts.  Every step
-// contains a sincos stage (the merged drift never rotates there), so these levels need no re-synchronisation.
+// A drift whose own largest angle needs more than degree kMaxRotDegree leaves that pair type stale, and the kick that
+// follows evaluates the table-driven sincos instead (degree 0 below); the decision is per drift and per pair type, so
+// from level 4 on the kernels are mixed: the short inner drifts rotate, the long ones (first the zeta pair, which
+// turns sqrt(2) faster) go through tsincos.  A pair type with a stale drift is recomputed in every step and needs no
+// re-synchronisation.
 constexpr double kLevelMaxD[10] = {0.0, 0.0104, 0.0147, 0.0354, 0.0500, 0.1166, 0.2192, 0.3570, 0.5400, 2.0};
 constexpr double kDegreeMaxAngle[9] = {0.0, 6.8e-5, 0.00293, 0.0208, 0.0708, 0.165, 0.310, 0.505, 0.750};
 
@@ -174,19 +184,19 @@ __host__ __device__ constexpr int rotation_degree() {
   return kDegreeMaxAngle[n] < t ? 0 : n;  // 0: the angle is too large for a rotation of degree <= kMaxRotDegree
 }
 
-// does the drift after kick s rotate the running pairs (true at levels 1-5, per drift at levels 6-9, never at 0)?
-template <int S, int LEVEL, int s>
+// Does the drift after kick s rotate the u and v pairs (ZETA = false) / the zeta pair (ZETA = true)?  Decided per
+// pair type: the zeta = 2z pair turns by sqrt(2) more than the other two, so it goes stale one level earlier.
+template <int S, int LEVEL, int s, bool ZETA>
 __host__ __device__ constexpr bool drift_rotates() {
   constexpr int cs = (s == S - 1) ? s : (s < S - 2 - s ? s : S - 2 - s);
-  return rotation_degree<S, LEVEL, cs, false>() > 0 && rotation_degree<S, LEVEL, cs, true>() > 0;
+  return rotation_degree<S, LEVEL, cs, ZETA>() > 0;
 }
-// Do all drifts of a step rotate?  Then the pairs live on rotations alone and are re-synchronised from the angles
-// every chunk; otherwise every step contains a kick that recomputes them from the angles (tsincos) and the kernel
-// needs the table.
-template <int S, int LEVEL, int s = 0>
+// Do all drifts of a step rotate this pair type?  Then it lives on rotations alone and is re-synchronised from the
+// angles every chunk; otherwise every step contains a kick that recomputes it from the angle (tsincos).
+template <int S, int LEVEL, bool ZETA, int s = 0>
 __host__ __device__ constexpr bool all_drifts_rotate() {
   if constexpr (s == S) return true;
-  else return drift_rotates<S, LEVEL, s>() && all_drifts_rotate<S, LEVEL, s + 1>();
+  else return drift_rotates<S, LEVEL, s, ZETA>() && all_drifts_rotate<S, LEVEL, ZETA, s + 1>();
 }
 
 // Everything a thread carries between stages.  Inside a block of `stride` steps the state is held in the
@@ -257,13 +267,15 @@ __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
   // the angle FMAs first: they depend only on the kick just done, and in the -O1 unit (source order) they fill
   // the latency of the kick's tail before the polynomial chains start (measured +0.8 to +1.6 %)
   drift_angles<TAN>(t, p.a_loop[cs], p.a2_loop[cs]);
-  if constexpr (drift_rotates<S, LEVEL, s>()) {
-    constexpr int nuv = rotation_degree<S, LEVEL, cs, false>(), nz = rotation_degree<S, LEVEL, cs, true>();
-    double g, m;
+  constexpr int nuv = rotation_degree<S, LEVEL, cs, false>(), nz = rotation_degree<S, LEVEL, cs, true>();
+  double g, m;
+  if constexpr (nuv > 0) {
     small_sincos<nuv>(t.pu, p.grot[cs], p.mrot[cs], g, m);
     rotate(t.su, t.cu, g, m);
     small_sincos<nuv>(t.pv, p.grot[cs], p.mrot[cs], g, m);
     rotate(t.sv, t.cv, g, m);
+  }
+  if constexpr (nz > 0) {
     small_sincos<nz>(t.pzt, p.grot[cs], p.mrot[cs], g, m);
     rotate(t.s2, t.c2, g, m);
   }
@@ -271,11 +283,15 @@ __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
 
 template <int S, bool TAN, int LEVEL>
 __device__ __forceinline__ void resync(Traj<TAN> &t) {
-  if constexpr (all_drifts_rotate<S, LEVEL>()) {  // otherwise a kick of every step recomputes the pairs anyway
+  // The merged drift is the longest of the step: if it rotates a pair type, every drift does, and that type lives on
+  // rotations alone (re-synchronised here); if not, the first kick of every step recomputes it from the angle.
+  static_assert(all_drifts_rotate<S, LEVEL, false>() == drift_rotates<S, LEVEL, S - 1, false>() &&
+                all_drifts_rotate<S, LEVEL, true>() == drift_rotates<S, LEVEL, S - 1, true>(), "drift ratios");
+  if constexpr (all_drifts_rotate<S, LEVEL, false>()) {
     sincos(t.u, t.su, t.cu);
     sincos(t.v, t.sv, t.cv);
-    sincos(t.zt, t.s2, t.c2);
   }
+  if constexpr (all_drifts_rotate<S, LEVEL, true>()) sincos(t.zt, t.s2, t.c2);
 }
 
 // kick of stage s in the rotated variables: P -= b grad H_p(X), dP -= b Hess H_p(X) dX (R3); b1 = b, b2 = 2b.
@@ -285,14 +301,15 @@ __device__ __forceinline__ void resync(Traj<TAN> &t) {
 //   dpv += b (F cos v dv - sin zeta sin v dzeta)
 //   dpz += b (-sin zeta (sin u du + sin v dv) + W cos zeta dzeta)
 // (the sum and difference of the x and y rows of SURVEY.md Appendix A.2, with dzeta = 2 dz).
-// FRESH: the running pairs are valid (the drift before this kick rotated them); otherwise they are evaluated here.
-template <bool TAN, bool FRESH>
-__device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2, const double2 *__restrict__ tab) {
-  if (!FRESH) {
+// FRESH_UV / FRESH_Z: the running pairs are valid (the drift before this kick rotated them); otherwise they are
+// evaluated here from the angles.
+template <bool TAN, bool FRESH_UV, bool FRESH_Z>
+__device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2, const TrigTable &tab) {
+  if (!FRESH_UV) {
     tsincos(tab, t.u, t.su, t.cu);
     tsincos(tab, t.v, t.sv, t.cv);
-    tsincos(tab, t.zt, t.s2, t.c2);
   }
+  if (!FRESH_Z) tsincos(tab, t.zt, t.s2, t.c2);
   const double F = fma(b1, t.c2, b1);  // b (1 + cos zeta)
   const double G2 = b2 * t.s2;         // 2 b sin zeta
   const double w = t.cu + t.cv;        // 2 cos x cos y
@@ -311,10 +328,11 @@ __device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2, const d
 
 // stages s, s+1, ..., S-1 of one step: kick_s then the drift after it
 template <int S, bool TAN, int LEVEL, int s>
-__device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p, const double2 *__restrict__ tab) {
+__device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p, const TrigTable &tab) {
   if constexpr (s < S) {
     // the drift before kick s is the one after kick s-1, or for s = 0 the merged drift that closed the last step
-    kick<TAN, drift_rotates<S, LEVEL, (s == 0 ? S - 1 : s - 1)>()>(t, p.b1[s], p.b2[s], tab);
+    constexpr int prev = (s == 0 ? S - 1 : s - 1);
+    kick<TAN, drift_rotates<S, LEVEL, prev, false>(), drift_rotates<S, LEVEL, prev, true>()>(t, p.b1[s], p.b2[s], tab);
     drift<S, TAN, LEVEL, s>(t, p);
     stages<S, TAN, LEVEL, s + 1>(t, p, tab);
   }
@@ -323,15 +341,17 @@ __device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p, c
 template <int S, bool TAN, int LEVEL>
 __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS(LEVEL))
     integrate_kernel(const __grid_constant__ IntegrateParams p) {
-  // the (sin, cos) table of tsincos, whole circle, 16 KB of shared memory per block (kernels with a stale drift only)
-  constexpr bool kUsesTable = !all_drifts_rotate<S, LEVEL>();
-  __shared__ double2 tab_s[kUsesTable ? kTab : 1];
+  // the (sin, cos) table of tsincos, 8 interleaved copies, 32 KB of shared memory (kernels with a stale drift only)
+  constexpr bool kUsesTable = !(all_drifts_rotate<S, LEVEL, false>() && all_drifts_rotate<S, LEVEL, true>());
+  __shared__ double2 tab_s[kUsesTable ? kTab * kTabCopies : 1];
   if constexpr (kUsesTable) {
-    for (int i = threadIdx.x; i < kTab; i += blockDim.x)
-      tab_s[i] = make_double2(aw_trig_table[2 * i], aw_trig_table[2 * i + 1]);
+    for (int i = threadIdx.x; i < kTab * kTabCopies; i += blockDim.x) {
+      const int e = i / kTabCopies;
+      tab_s[i] = make_double2(aw_trig_table[2 * e], aw_trig_table[2 * e + 1]);
+    }
     __syncthreads();
   }
-  const double2 *tab = tab_s;
+  const TrigTable tab = {reinterpret_cast<const char *>(tab_s), (threadIdx.x & (kTabCopies - 1)) * 16u};
   // blocks of 32, 64 or 128 threads (launch_one): the arithmetic is per trajectory, so the result does not depend on it
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= p.n) return;
