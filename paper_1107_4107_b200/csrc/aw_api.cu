@@ -318,10 +318,15 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
   p.a_open = a[0];
   for (int k = 1; k < S; ++k) p.a_loop[k - 1] = a[k];
   p.a_loop[S - 1] = a[S] + a[0];
-  for (int k = 0; k < S; ++k) { p.b1[k] = b[k]; p.b2[k] = 2.0 * b[k]; }
+  if (b[S - 1] != b[0]) return AW_ESTATE;  // palindromic: the outer stages share the weight the zeta pair is scaled by
   for (int k = 0; k < S; ++k) {
-    p.a2_loop[k] = 2.0 * p.a_loop[k];
-    rotation_coefficients(p.a_loop[k], p.grot[k], p.mrot[k]);
+    p.b2[k] = 2.0 * b[k];
+    p.rho[k] = (b[0] != 0.0) ? b[k] / b[0] : 0.0;
+    p.b4[k] = 4.0 * b[k];
+    p.rho2[k] = 2.0 * p.rho[k];
+    p.ah_loop[k] = 0.5 * p.a_loop[k];
+    rotation_coefficients(p.ah_loop[k], p.grot_uv[k], p.mrot_uv[k]);
+    rotation_coefficients(p.a_loop[k], p.grot_z[k], p.mrot_z[k]);
   }
   p.eps = s->eps;
   if (s->survive != 0 && s->survive != 1) return AW_EINVAL;

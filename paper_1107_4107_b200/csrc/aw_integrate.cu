@@ -201,21 +201,25 @@ __host__ __device__ constexpr bool all_drifts_rotate() {
 
 // Everything a thread carries between stages.  Inside a block of `stride` steps the state is held in the
 // rotated and scaled variables
-//     u = x + y,  v = x - y,  zeta = 2 z,   pu = px + py,  pv = px - py,  pzeta = 2 pz
-// (tangent vector: du, dv, dzeta = 2 dz, dpu, dpv, and dpz itself), in which
+//     u = x + y,  v = x - y,  zeta = 2 z,   pu = 2 (px + py),  pv = 2 (px - py),  pzt = 2 pz  (4 pz for S = 7, below)
+// (tangent vector: du, dv, dzt = 2 dz, dpu = 2 (dpx + dpy), dpv = 2 (dpx - dpy), dpz = 2 dpz), in which
 //     H_p = (cos u + cos v)(1 + cos zeta)/2:
-// the kick needs no products of the x and y functions,
-//     pu += b F sin u,  pv += b F sin v,  pzeta += 2 b (cos u + cos v) sin zeta,        F = 1 + cos zeta,
-// the tangent kick is seven multiply-adds instead of nine (kick()), and all three angles drift with the
-// same constant (u += a pu, v += a pv, zeta += a pzeta), so one set of rotation coefficients serves the three
-// pairs and every constant of the loop fits the uniform registers.  The change of variables is linear, so
-// the map is the same map; halving and doubling are exact; the state is converted back to (x, y, z) for
-// every checkpoint and for the store.
+// the kick needs no products of the x and y functions, the tangent kick is seven multiply-adds instead of nine
+// (kick()), and with every momentum-like variable doubled the kick's coefficients are exactly the quantities the
+// carried pairs provide (no constant multiplies on the native stages, see kick()).  u and v then advance with a/2
+// per unit of pu, pv and zeta with a per unit of pzt, so the rotations take two coefficient sets (A = a/2 and A = a).
+// The 7-stage scheme has four distinct drift constants, and two sets for each do not fit the uniform registers
+// (ptxas then reloads constants inside the loop: +45..57 issue cycles per step); there pzt = 4 pz, so that zeta too
+// advances with a/2 per unit of pzt and one set serves the three pairs, at the price of a factor 2 in the pzt kick.
+// The change of variables is linear, so the map is the same map; halving and doubling are exact; the state is
+// converted back to (x, y, z) for every checkpoint and for the store.
 template <bool TAN>
 struct Traj {
   double u, v, zt, pu, pv, pzt;
   double du, dv, dzt, dpu, dpv, dpz;
-  double su, cu, sv, cv, s2, c2;  // sin u, cos u, sin v, cos v, sin zeta, cos zeta (LEVEL >= 1)
+  // sin u, cos u, sin v, cos v; (s2, c2) = kz (sin zeta, cos zeta) with kz = 2 b_0 when the zeta pair lives on
+  // rotations (every drift rotates it), kz = 1 when a kick of every step recomputes it from the angle
+  double su, cu, sv, cv, s2, c2;
 };
 
 // (x, y) -> (x + y, x - y) and back, in place, for every pair of the first two degrees of freedom
@@ -224,38 +228,46 @@ __device__ __forceinline__ void to_sum_diff(double &a, double &b) {
   a = s;
   b = d;
 }
-__device__ __forceinline__ void from_sum_diff(double &a, double &b) {
-  const double x = 0.5 * (a + b), y = 0.5 * (a - b);
+__device__ __forceinline__ void from_sum_diff(double &a, double &b, double half) {
+  const double x = half * (a + b), y = half * (a - b);
   a = x;
   b = y;
 }
-template <bool TAN>
+// pzt = kPzScale<S> pz
+template <int S> constexpr double kPzScale = (S == 3) ? 2.0 : 4.0;
+
+template <int S, bool TAN>
 __device__ __forceinline__ void rotate_in(Traj<TAN> &t) {
   to_sum_diff(t.u, t.v);
   to_sum_diff(t.pu, t.pv);
+  t.pu *= 2.0; t.pv *= 2.0;
   t.zt *= 2.0;
-  t.pzt *= 2.0;
-  if (TAN) { to_sum_diff(t.du, t.dv); to_sum_diff(t.dpu, t.dpv); t.dzt *= 2.0; }
+  t.pzt *= kPzScale<S>;
+  if (TAN) {
+    to_sum_diff(t.du, t.dv); to_sum_diff(t.dpu, t.dpv);
+    t.dpu *= 2.0; t.dpv *= 2.0; t.dzt *= 2.0; t.dpz *= 2.0;
+  }
 }
-// The momenta come back as px = px0 + ((pu - pu0) + (pv - pv0))/2 with (px0, py0) the values the block started
-// from and pu0 = px0 + py0, pv0 = px0 - py0 as rotate_in rounded them: the differences are exact (or nearly),
+// The momenta come back as px = px0 + ((pu - pu0) + (pv - pv0))/4 with (px0, py0) the values the block started
+// from and pu0 = 2 (px0 + py0), pv0 = 2 (px0 - py0) as rotate_in rounded them: the differences are exact (or nearly),
 // so the rounding of the forward conversion cancels and P stays bit-constant when the kicks vanish (eps = 0).
-template <bool TAN>
+template <int S, bool TAN>
 __device__ __forceinline__ void rotate_out(Traj<TAN> &t, double px0, double py0) {
-  from_sum_diff(t.u, t.v);
-  const double du = t.pu - (px0 + py0), dv = t.pv - (px0 - py0);
-  t.pu = fma(0.5, du + dv, px0);
-  t.pv = fma(0.5, du - dv, py0);
+  from_sum_diff(t.u, t.v, 0.5);
+  const double du = t.pu - 2.0 * (px0 + py0), dv = t.pv - 2.0 * (px0 - py0);
+  t.pu = fma(0.25, du + dv, px0);
+  t.pv = fma(0.25, du - dv, py0);
   t.zt *= 0.5;
-  t.pzt *= 0.5;
-  if (TAN) { from_sum_diff(t.du, t.dv); from_sum_diff(t.dpu, t.dpv); t.dzt *= 0.5; }
+  t.pzt *= 1.0 / kPzScale<S>;
+  if (TAN) { from_sum_diff(t.du, t.dv, 0.5); from_sum_diff(t.dpu, t.dpv, 0.25); t.dzt *= 0.5; t.dpz *= 0.5; }
 }
 
-// angles (and tangent angles) only: X += a P; a2 = 2a (dzeta = 2 dz advances with dpz)
-template <bool TAN>
-__device__ __forceinline__ void drift_angles(Traj<TAN> &t, double a, double a2) {
-  t.u = fma(a, t.pu, t.u); t.v = fma(a, t.pv, t.v); t.zt = fma(a, t.pzt, t.zt);
-  if (TAN) { t.du = fma(a, t.dpu, t.du); t.dv = fma(a, t.dpv, t.dv); t.dzt = fma(a2, t.dpz, t.dzt); }
+// angles (and tangent angles) only: X += a P with ah = a/2 for the u, v variables (momenta doubled), a for dzt (and
+// for zeta when pzt = 2 pz; a/2 when pzt = 4 pz)
+template <int S, bool TAN>
+__device__ __forceinline__ void drift_angles(Traj<TAN> &t, double ah, double a) {
+  t.u = fma(ah, t.pu, t.u); t.v = fma(ah, t.pv, t.v); t.zt = fma(S == 3 ? a : ah, t.pzt, t.zt);
+  if (TAN) { t.du = fma(ah, t.dpu, t.du); t.dv = fma(ah, t.dpv, t.dv); t.dzt = fma(a, t.dpz, t.dzt); }
 }
 
 // drift after kick s of the step loop: angles and, for LEVEL >= 1, the running pairs.  The stage lists are
@@ -266,23 +278,28 @@ __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
   constexpr int cs = (s == S - 1) ? s : (s < S - 2 - s ? s : S - 2 - s);
   // the angle FMAs first: they depend only on the kick just done, and in the -O1 unit (source order) they fill
   // the latency of the kick's tail before the polynomial chains start (measured +0.8 to +1.6 %)
-  drift_angles<TAN>(t, p.a_loop[cs], p.a2_loop[cs]);
+  drift_angles<S, TAN>(t, p.ah_loop[cs], p.a_loop[cs]);
   constexpr int nuv = rotation_degree<S, LEVEL, cs, false>(), nz = rotation_degree<S, LEVEL, cs, true>();
   double g, m;
   if constexpr (nuv > 0) {
-    small_sincos<nuv>(t.pu, p.grot[cs], p.mrot[cs], g, m);
+    small_sincos<nuv>(t.pu, p.grot_uv[cs], p.mrot_uv[cs], g, m);
     rotate(t.su, t.cu, g, m);
-    small_sincos<nuv>(t.pv, p.grot[cs], p.mrot[cs], g, m);
+    small_sincos<nuv>(t.pv, p.grot_uv[cs], p.mrot_uv[cs], g, m);
     rotate(t.sv, t.cv, g, m);
   }
   if constexpr (nz > 0) {
-    small_sincos<nz>(t.pzt, p.grot[cs], p.mrot[cs], g, m);
+    if constexpr (S == 3) small_sincos<nz>(t.pzt, p.grot_z[cs], p.mrot_z[cs], g, m);     // A = a,   pzt = 2 pz
+    else small_sincos<nz>(t.pzt, p.grot_uv[cs], p.mrot_uv[cs], g, m);                    // A = a/2, pzt = 4 pz
     rotate(t.s2, t.c2, g, m);
   }
 }
 
+// Is the zeta pair carried scaled by 2 b_0 (it lives on rotations, which are linear) or plain?
+template <int S, int LEVEL>
+__host__ __device__ constexpr bool zeta_pair_scaled() { return all_drifts_rotate<S, LEVEL, true>(); }
+
 template <int S, bool TAN, int LEVEL>
-__device__ __forceinline__ void resync(Traj<TAN> &t) {
+__device__ __forceinline__ void resync(Traj<TAN> &t, const IntegrateParams &p) {
   // The merged drift is the longest of the step: if it rotates a pair type, every drift does, and that type lives on
   // rotations alone (re-synchronised here); if not, the first kick of every step recomputes it from the angle.
   static_assert(all_drifts_rotate<S, LEVEL, false>() == drift_rotates<S, LEVEL, S - 1, false>() &&
@@ -291,35 +308,47 @@ __device__ __forceinline__ void resync(Traj<TAN> &t) {
     sincos(t.u, t.su, t.cu);
     sincos(t.v, t.sv, t.cv);
   }
-  if constexpr (all_drifts_rotate<S, LEVEL, true>()) sincos(t.zt, t.s2, t.c2);
+  if constexpr (zeta_pair_scaled<S, LEVEL>()) {
+    sincos(t.zt, t.s2, t.c2);
+    t.s2 *= p.b2[0];
+    t.c2 *= p.b2[0];
+  }
 }
 
-// kick of stage s in the rotated variables: P -= b grad H_p(X), dP -= b Hess H_p(X) dX (R3); b1 = b, b2 = 2b.
-// With F = 1 + cos zeta, W = cos u + cos v:
-//   pu += b F sin u,   pv += b F sin v,   pzeta += 2 b W sin zeta
-//   dpu += b (F cos u du - sin zeta sin u dzeta)
-//   dpv += b (F cos v dv - sin zeta sin v dzeta)
-//   dpz += b (-sin zeta (sin u du + sin v dv) + W cos zeta dzeta)
-// (the sum and difference of the x and y rows of SURVEY.md Appendix A.2, with dzeta = 2 dz).
+// kick of stage s in the rotated variables: P -= b grad H_p(X), dP -= b Hess H_p(X) dX (R3).  In natural variables,
+// with W = cos u + cos v (the sum and difference of the x and y rows of SURVEY.md Appendix A.2, dzeta = 2 dz):
+//   d(px+py) = b (1 + cos zeta) sin u,   d(px-py) = b (1 + cos zeta) sin v,   d(pz) = b W sin zeta
+//   d(dpx+dpy) = b ((1 + cos zeta) cos u du - sin zeta sin u dzeta),   likewise v
+//   d(dpz) = b (-sin zeta (sin u du + sin v dv) + W cos zeta dzeta)
+// With every momentum-like variable doubled and (Sz, Cz) = 2b (sin zeta, cos zeta), F = Cz + 2b:
+//   pu += F su,  pv += F sv,  pzt += W Sz
+//   dpu += (F cu) du - (Sz su) dzt,  dpv += (F cv) dv - (Sz sv) dzt,  dpz += -(Sz su) du - (Sz sv) dv + (Cz W) dzt
+// i.e. 2 adds + 5 products + 10 multiply-adds with no constant multiplies at all when the carried pair already is
+// (Sz, Cz) — ZMODE 0: the pair lives on rotations scaled by 2 b_0 and this stage's weight is b_0 (the first and
+// last stage of the palindromic schemes).  ZMODE 1: scaled pair, other weight: Sz = rho s2, Cz = rho c2 with
+// rho = b_s / b_0, folded as F = fma(rho, c2, 2b), W' = rho W.  ZMODE 2: plain pair (recomputed by tsincos in every
+// step): the same with kz = 2 b_s in place of rho.
+// PZ4 (the 7-stage scheme): pzt = 4 pz takes 2 W Sz, i.e. its own product with the constant 2 kz (2 when ZMODE 0).
 // FRESH_UV / FRESH_Z: the running pairs are valid (the drift before this kick rotated them); otherwise they are
 // evaluated here from the angles.
-template <bool TAN, bool FRESH_UV, bool FRESH_Z>
-__device__ __forceinline__ void kick(Traj<TAN> &t, double b1, double b2, const TrigTable &tab) {
+template <bool TAN, bool FRESH_UV, bool FRESH_Z, int ZMODE, bool PZ4>
+__device__ __forceinline__ void kick(Traj<TAN> &t, double b2, double kz, double kz2, const TrigTable &tab) {
   if (!FRESH_UV) {
     tsincos(tab, t.u, t.su, t.cu);
     tsincos(tab, t.v, t.sv, t.cv);
   }
   if (!FRESH_Z) tsincos(tab, t.zt, t.s2, t.c2);
-  const double F = fma(b1, t.c2, b1);  // b (1 + cos zeta)
-  const double G2 = b2 * t.s2;         // 2 b sin zeta
-  const double w = t.cu + t.cv;        // 2 cos x cos y
+  const double W = t.cu + t.cv;                                   // 2 cos x cos y
+  const double F = ZMODE == 0 ? t.c2 + b2 : fma(kz, t.c2, b2);    // 2 b (1 + cos zeta)
+  const double Wk = (ZMODE == 0 || (PZ4 && !TAN)) ? W : kz * W;   // feeds e5 (and pzt unless PZ4)
+  const double Wz = !PZ4 ? Wk : (ZMODE == 0 ? 2.0 * W : kz2 * W);
   t.pu = fma(t.su, F, t.pu);
   t.pv = fma(t.sv, F, t.pv);
-  t.pzt = fma(w, G2, t.pzt);
+  t.pzt = fma(Wz, t.s2, t.pzt);
   if (TAN) {
-    const double G = b1 * t.s2;  // b sin zeta
-    const double a1 = F * t.cu, a2 = F * t.cv, k1 = G * t.su, k2 = G * t.sv;
-    const double e5 = w * (b1 * t.c2);  // b (cos u + cos v) cos zeta
+    const double Sz = ZMODE == 0 ? t.s2 : kz * t.s2;              // 2 b sin zeta
+    const double a1 = F * t.cu, a2 = F * t.cv, k1 = Sz * t.su, k2 = Sz * t.sv;
+    const double e5 = t.c2 * Wk;                                  // 2 b cos zeta W
     t.dpu = fma(a1, t.du, t.dpu); t.dpv = fma(a2, t.dv, t.dpv); t.dpz = fma(e5, t.dzt, t.dpz);
     t.dpu = fma(-k1, t.dzt, t.dpu); t.dpz = fma(-k1, t.du, t.dpz);
     t.dpv = fma(-k2, t.dzt, t.dpv); t.dpz = fma(-k2, t.dv, t.dpz);
@@ -332,7 +361,9 @@ __device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p, c
   if constexpr (s < S) {
     // the drift before kick s is the one after kick s-1, or for s = 0 the merged drift that closed the last step
     constexpr int prev = (s == 0 ? S - 1 : s - 1);
-    kick<TAN, drift_rotates<S, LEVEL, prev, false>(), drift_rotates<S, LEVEL, prev, true>()>(t, p.b1[s], p.b2[s], tab);
+    constexpr int zmode = !zeta_pair_scaled<S, LEVEL>() ? 2 : ((s == 0 || s == S - 1) ? 0 : 1);
+    kick<TAN, drift_rotates<S, LEVEL, prev, false>(), drift_rotates<S, LEVEL, prev, true>(), zmode, S != 3>(
+        t, p.b2[s], zmode == 2 ? p.b2[s] : p.rho[s], zmode == 2 ? p.b4[s] : p.rho2[s], tab);
     drift<S, TAN, LEVEL, s>(t, p);
     stages<S, TAN, LEVEL, s + 1>(t, p, tab);
   }
@@ -341,7 +372,7 @@ __device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p, c
 template <int S, bool TAN, int LEVEL>
 __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS(LEVEL))
     integrate_kernel(const __grid_constant__ IntegrateParams p) {
-  // the (sin, cos) table of tsincos, 8 interleaved copies, 32 KB of shared memory (kernels with a stale drift only)
+  // the (sin, cos) table of tsincos, 4 interleaved copies, 32 KB of shared memory (kernels with a stale drift only)
   constexpr bool kUsesTable = !(all_drifts_rotate<S, LEVEL, false>() && all_drifts_rotate<S, LEVEL, true>());
   __shared__ double2 tab_s[kUsesTable ? kTab * kTabCopies : 1];
   if constexpr (kUsesTable) {
@@ -370,9 +401,9 @@ __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS(LEVEL))
 
   for (int chk = 0; chk < p.nchk; ++chk) {
     const double px0 = t.pu, py0 = t.pv;
-    rotate_in<TAN>(t);                              // (x, y, z) -> (u, v, zeta)
-    drift_angles<TAN>(t, p.a_open, 2.0 * p.a_open);  // opening drift of the block
-    resync<S, TAN, LEVEL>(t);        // pairs from the angles: the same values a new launch would start from
+    rotate_in<S, TAN>(t);                           // (x, y, z) -> (u, v, zeta)
+    drift_angles<S, TAN>(t, 0.5 * p.a_open, p.a_open);  // opening drift of the block
+    resync<S, TAN, LEVEL>(t, p);     // pairs from the angles: the same values a new launch would start from
 
 #pragma unroll 1
     for (int rem = p.stride; rem > 0;) {
@@ -380,10 +411,10 @@ __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS(LEVEL))
       rem -= m;
 #pragma unroll 1
       for (int i = m; i > 0; --i) stages<S, TAN, LEVEL, 0>(t, p, tab);
-      if (rem > 0) resync<S, TAN, LEVEL>(t);
+      if (rem > 0) resync<S, TAN, LEVEL>(t, p);
     }
-    drift_angles<TAN>(t, -p.a_open, -2.0 * p.a_open);  // last merged drift -> closing drift of the block
-    rotate_out<TAN>(t, px0, py0);                      // (u, v, zeta) -> (x, y, z)
+    drift_angles<S, TAN>(t, -0.5 * p.a_open, -p.a_open);  // last merged drift -> closing drift of the block
+    rotate_out<S, TAN>(t, px0, py0);                   // (u, v, zeta) -> (x, y, z)
     double &x = t.u, &y = t.v, &z = t.zt, &px = t.pu, &py = t.pv, &pz = t.pzt;
     double &dx = t.du, &dy = t.dv, &dz = t.dzt, &dpx = t.dpu, &dpy = t.dpv;
 

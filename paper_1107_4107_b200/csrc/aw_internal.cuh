@@ -26,16 +26,21 @@ struct IntegrateParams {
   int32_t level;   // trigonometry variant picked on the host from the largest drift angle (aw_integrate.cu)
   double a_open;   // a_1 (= a_{S+1}): angle drift that opens a block of `stride` steps; the block is closed by
                    // the angle drift -a_open, which takes the last merged drift back to the step boundary
-  double a2_loop[kMaxStages]; // 2 a_loop[s] (exact): tangent drift of dzeta = 2 dz with dpz
-  double a_loop[kMaxStages];  // drift after kick s (s = 0..S-1): a_2 .. a_S, then a_{S+1} + a_1 (closing drift
-                              // of one step merged with the opening drift of the next)
-  // Rotation of the running (sin, cos) pairs through the drift after kick s by the angle d = A p, A = a_loop[s],
-  // p = pu, pv or pzeta, as polynomials in z = p^2 (aw_integrate.cu):
-  //   sin d = p (G[0] + G[1] z + ...),  G[i] = (-1)^i A^(2i+1) / (2i+1)!      (G[0] = A exactly)
-  //   cos d - 1 = z (M[0] + M[1] z + ...),  M[i] = (-1)^(i+1) A^(2i+2) / (2i+2)!
-  double grot[kMaxStages][kTrigTerms + 1], mrot[kMaxStages][kTrigTerms];
-  double b1[kMaxStages];     // b_s
+  // Drift after kick s (s = 0..S-1): a_2 .. a_S, then a_{S+1} + a_1 (closing drift of one step merged with the
+  // opening drift of the next).  The kernel's momentum-like variables are twice the natural ones (aw_integrate.cu,
+  // struct Traj), so u, v (and du, dv) advance with a/2 and zeta = 2z (and dzeta) with a.
+  double a_loop[kMaxStages];   // a: zeta += a pzeta, dzeta += a Q
+  double ah_loop[kMaxStages];  // a / 2 (exact): u += (a/2) pu', du += (a/2) Pu
+  // Rotation of the running (sin, cos) pairs through the drift after kick s by the angle d = A p as polynomials in
+  // z = p^2 (aw_integrate.cu):   sin d = p (G[0] + G[1] z + ...),  G[i] = (-1)^i A^(2i+1) / (2i+1)!   (G[0] = A exactly)
+  //                              cos d - 1 = z (M[0] + M[1] z + ...),  M[i] = (-1)^(i+1) A^(2i+2) / (2i+2)!
+  // one set for the u and v pairs (A = a/2, p = pu', pv') and one for the zeta pair (A = a, p = pzeta)
+  double grot_uv[kMaxStages][kTrigTerms + 1], mrot_uv[kMaxStages][kTrigTerms];
+  double grot_z[kMaxStages][kTrigTerms + 1], mrot_z[kMaxStages][kTrigTerms];
   double b2[kMaxStages];     // 2 b_s
+  double rho[kMaxStages];    // b_s / b_0 (0 if b_0 = 0): the zeta pair is carried scaled by 2 b_0 (aw_integrate.cu, kick)
+  double b4[kMaxStages];     // 4 b_s  and
+  double rho2[kMaxStages];   // 2 b_s / b_0: the same two factors for the 7-stage scheme, whose pzt is 4 pz
   double eps;
   int32_t survive;  // survivor filter (R25): 1 = test (px, py) against surv[] at every checkpoint
   int32_t block;    // threads per block (32, 64 or 128)
