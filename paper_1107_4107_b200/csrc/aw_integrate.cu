@@ -349,9 +349,13 @@ __device__ __forceinline__ void kick(Traj<TAN> &t, double b2, double kz, double 
     const double Sz = ZMODE == 0 ? t.s2 : kz * t.s2;              // 2 b sin zeta
     const double a1 = F * t.cu, a2 = F * t.cv, k1 = Sz * t.su, k2 = Sz * t.sv;
     const double e5 = t.c2 * Wk;                                  // 2 b cos zeta W
-    t.dpu = fma(a1, t.du, t.dpu); t.dpv = fma(a2, t.dv, t.dpv); t.dpz = fma(e5, t.dzt, t.dpz);
-    t.dpu = fma(-k1, t.dzt, t.dpu); t.dpz = fma(-k1, t.du, t.dpz);
-    t.dpv = fma(-k2, t.dzt, t.dpv); t.dpz = fma(-k2, t.dv, t.dpz);
+    // Seven all-register multiply-adds, grouped by the operand they share in the same slot (du, dv, dzt): in the -O1
+    // unit ptxas keeps this order, and the operand-reuse cache then serves the repeated operand (a DFMA with three
+    // fresh register operands issues in 3 cycles instead of 2).  Measured on configs[3] against five other orders:
+    // +1.0 % over the round-1 order (a1, a2, e5 first), the others within -0.8 .. +0.8 %.
+    t.dpu = fma(a1, t.du, t.dpu); t.dpz = fma(-k1, t.du, t.dpz);
+    t.dpv = fma(a2, t.dv, t.dpv); t.dpz = fma(-k2, t.dv, t.dpz);
+    t.dpu = fma(-k1, t.dzt, t.dpu); t.dpv = fma(-k2, t.dzt, t.dpv); t.dpz = fma(e5, t.dzt, t.dpz);
   }
 }
 
