@@ -24,8 +24,11 @@
 // vs finite differences, pendulum reduction vs the complete elliptic integral, invariant subspaces
 // (P:79), shell layer, IC energy, histogram brute force; averaged velocity vs eps=0 closed
 // form, vs an unwrapped brute-force run and vs the pendulum rotation frequency 2 pi / T(h); central
-// projection on a hand case; survivor filter vs a stepwise brute force.  No function here is
-// "parity unpinned" except where DESIGN.md §3 says so (the paper's figures and its dE<1e-8 remark).
+// projection on a hand case; survivor filter vs a stepwise brute force; the indicator kinds and masks on a
+// hand-made table (strict FLI > thr, 255 / NaN for every status != 1); slices by global index against the whole
+// and the cell-centre definition; the Gaussian cloud's Rayleigh law; cloud resampling against plain ensembles of the
+// attempt seeds.  tests/test_oracle_sanitizers.py runs this file under -fsanitize=address,undefined.  No function
+// here is "parity unpinned" except where DESIGN.md §3 says so (the paper's figures and its dE<1e-8 remark).
 
 #include <cmath>
 #include <cstdint>
