@@ -79,14 +79,18 @@ __device__ __forceinline__ double wrap_angle(double x, int &turns) {
 
 // g = sin(A p), m = cos(A p) - 1 as p G(z), z M(z), z = p^2: N + (N-1) FMA with uniform-register coefficients,
 // 3 DMUL.  Truncation: |d|^(2N+3)/(2N+3)! in g, |d|^(2N+2)/(2N+2)! in m (d = A p).
+// G[0] = A exactly, and A is the drift constant the angle FMAs of the same drift already hold in a uniform register:
+// it is passed separately so that ptxas keeps ONE copy (the loop's constants do not all fit the uniform registers; the
+// overflow lives in ordinary registers, where a polynomial FMA becomes a three-register one).
 template <int N>
-__device__ __forceinline__ void small_sincos(double p, const double (&G)[kTrigTerms + 1],
+__device__ __forceinline__ void small_sincos(double p, double A, const double (&G)[kTrigTerms + 1],
                                              const double (&M)[kTrigTerms], double &g, double &m) {
   static_assert(N >= 1 && N <= kTrigTerms, "degree");
   const double z = p * p;
   double pg = G[N], pm = M[N - 1];
 #pragma unroll
-  for (int i = N - 1; i >= 0; --i) pg = fma(pg, z, G[i]);
+  for (int i = N - 1; i >= 1; --i) pg = fma(pg, z, G[i]);
+  pg = fma(pg, z, A);
 #pragma unroll
   for (int i = N - 2; i >= 0; --i) pm = fma(pm, z, M[i]);
   g = p * pg;
@@ -282,14 +286,14 @@ __device__ __forceinline__ void drift(Traj<TAN> &t, const IntegrateParams &p) {
   constexpr int nuv = rotation_degree<S, LEVEL, cs, false>(), nz = rotation_degree<S, LEVEL, cs, true>();
   double g, m;
   if constexpr (nuv > 0) {
-    small_sincos<nuv>(t.pu, p.grot_uv[cs], p.mrot_uv[cs], g, m);
+    small_sincos<nuv>(t.pu, p.ah_loop[cs], p.grot_uv[cs], p.mrot_uv[cs], g, m);
     rotate(t.su, t.cu, g, m);
-    small_sincos<nuv>(t.pv, p.grot_uv[cs], p.mrot_uv[cs], g, m);
+    small_sincos<nuv>(t.pv, p.ah_loop[cs], p.grot_uv[cs], p.mrot_uv[cs], g, m);
     rotate(t.sv, t.cv, g, m);
   }
   if constexpr (nz > 0) {
-    if constexpr (S == 3) small_sincos<nz>(t.pzt, p.grot_z[cs], p.mrot_z[cs], g, m);     // A = a,   pzt = 2 pz
-    else small_sincos<nz>(t.pzt, p.grot_uv[cs], p.mrot_uv[cs], g, m);                    // A = a/2, pzt = 4 pz
+    if constexpr (S == 3) small_sincos<nz>(t.pzt, p.a_loop[cs], p.grot_z[cs], p.mrot_z[cs], g, m);    // A = a,   pzt = 2 pz
+    else small_sincos<nz>(t.pzt, p.ah_loop[cs], p.grot_uv[cs], p.mrot_uv[cs], g, m);                // A = a/2, pzt = 4 pz
     rotate(t.s2, t.c2, g, m);
   }
 }
