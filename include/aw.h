@@ -179,7 +179,9 @@ AW_API int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps,
  * steps.  The bound is max(s->E, s->Emax) and it is ENFORCED: every call first runs one elementwise kernel that
  * evaluates each live trajectory's H(X,P) and compares it with the largest energy the chosen level (and the angle
  * range of R7) supports; above it the trajectory gets AW_ST_RANGE and is not touched (P^2 <= 2(H + 2|eps|)
- * along the whole orbit, so the check before the first step covers every step).  Call aw_bound_energy after uploading a state whose
+ * along the whole orbit, so the check before the first step covers every step).  The flag is a status like any other:
+ * to integrate such a trajectory after all, set its status byte back to AW_ST_LIVE and raise the bound (aw_bound_energy
+ * considers live trajectories only).  Call aw_bound_energy after uploading a state whose
  * energy the struct does not know.  If the drift angle can exceed
  * 0.357 rad the kernel is mixed (levels 8 and 9, up to 0.54 and 2 rad): the scheme's shorter drifts still rotate the
  * pairs, the long ones are followed by the device sincos; beyond 2 rad, or with s->trig == 1, the device sincos is evaluated at

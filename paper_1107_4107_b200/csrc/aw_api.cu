@@ -192,6 +192,20 @@ static VelocityArgs velocity_args(const aw_state *s) {
   return v;
 }
 
+// what aw_integrate checks about its scalar arguments and the struct's switches (shared with the *_map_host calls,
+// which must refuse a bad call before the first copy is enqueued)
+static int validate_integrate_args(const aw_state *s, int64_t steps, double dt, int64_t stride) {
+  if (steps < 0 || stride <= 0 || steps % stride != 0) return AW_EINVAL;
+  if (!(dt != 0.0) || !std::isfinite(dt)) return AW_EINVAL;
+  if (s->order != 4 && s->order != 6) return AW_ESTATE;
+  if (!std::isfinite(s->E) || !std::isfinite(s->eps)) return AW_ESTATE;
+  if (stride > 0x7fffffff) return AW_ERANGE;
+  if (s->survive != 0 && s->survive != 1) return AW_EINVAL;
+  if (s->survive && !(s->surv_hi_x > s->surv_lo_x && s->surv_hi_y > s->surv_lo_y)) return AW_EINVAL;
+  if (s->block != 0 && s->block != 32 && s->block != 64 && s->block != 128) return AW_EINVAL;
+  return AW_OK;
+}
+
 }  // namespace aw
 
 using namespace aw;
@@ -296,12 +310,9 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
   if (!s) return AW_EINVAL;
   int rc = check_planes(s);
   if (rc != AW_OK) return rc;
-  if (n != s->n || steps < 0 || stride <= 0 || steps % stride != 0) return AW_EINVAL;
-  if (!(dt != 0.0) || !std::isfinite(dt)) return AW_EINVAL;
-  if (!s->ready || (s->order != 4 && s->order != 6)) return AW_ESTATE;
-  if (!std::isfinite(s->E) || !std::isfinite(s->eps)) return AW_ESTATE;
-  if (stride > 0x7fffffff) return AW_ERANGE;
-  if (s->block != 0 && s->block != 32 && s->block != 64 && s->block != 128) return AW_EINVAL;
+  if (n != s->n) return AW_EINVAL;
+  if ((rc = validate_integrate_args(s, steps, dt, stride)) != AW_OK) return rc;
+  if (!s->ready) return AW_ESTATE;
   const double vmax = std::sqrt(2.0 * (energy_bound(s) + 2.0 * std::fabs(s->eps)));
   if (!((double)stride * std::fabs(dt) * vmax < 1024.0)) return AW_ERANGE;
   if (steps == 0 || n == 0) return AW_OK;
@@ -329,10 +340,8 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
     rotation_coefficients(p.a_loop[k], p.grot_z[k], p.mrot_z[k]);
   }
   p.eps = s->eps;
-  if (s->survive != 0 && s->survive != 1) return AW_EINVAL;
   p.survive = s->survive;
   p.surv[0] = s->surv_lo_x; p.surv[1] = s->surv_hi_x; p.surv[2] = s->surv_lo_y; p.surv[3] = s->surv_hi_y;
-  if (s->survive && !(s->surv_hi_x > s->surv_lo_x && s->surv_hi_y > s->surv_lo_y)) return AW_EINVAL;
   // running-(sin, cos) variant: degree from the largest drift angle, re-synchronisation cadence from stride
   double amax = std::fabs(p.a_open);
   for (int k = 0; k < S; ++k) amax = std::fmax(amax, std::fabs(p.a_loop[k]));
@@ -487,18 +496,6 @@ int synced(cudaStream_t st, int rc) {
     cudaError_t e_ = (call);                                                      \
     if (e_ != cudaSuccess) { cudaStreamSynchronize(st); return ::aw::cuda_fail(e_); } \
   } while (0)
-
-int validate_integrate_args(const aw_state *s, int64_t steps, double dt, int64_t stride) {
-  if (steps < 0 || stride <= 0 || steps % stride != 0) return AW_EINVAL;
-  if (!(dt != 0.0) || !std::isfinite(dt)) return AW_EINVAL;
-  if (s->order != 4 && s->order != 6) return AW_ESTATE;
-  if (!std::isfinite(s->E) || !std::isfinite(s->eps)) return AW_ESTATE;
-  if (stride > 0x7fffffff) return AW_ERANGE;
-  if (s->survive != 0 && s->survive != 1) return AW_EINVAL;
-  if (s->survive && !(s->surv_hi_x > s->surv_lo_x && s->surv_hi_y > s->surv_lo_y)) return AW_EINVAL;
-  if (s->block != 0 && s->block != 32 && s->block != 64 && s->block != 128) return AW_EINVAL;
-  return AW_OK;
-}
 
 int validate_hist_args(int32_t gx, int32_t gy, double lo, double hi, const void *hist_dev) {
   if (gx <= 0 || gy <= 0 || !(hi > lo) || !std::isfinite(lo) || !std::isfinite(hi)) return AW_EINVAL;
