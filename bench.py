@@ -243,6 +243,18 @@ def measured_traffic(build_hash, kernel, config, steps_per_launch):
     return None, None
 
 
+def ptxas_report(kernel_tag):
+    """(registers per thread, spill bytes) ptxas printed for the kernel when libaw.so was built (build/ptxas.log)."""
+    import re
+    try:
+        log = open(os.path.join(ROOT, "paper_1107_4107_b200", "build", "ptxas.log")).read()
+    except OSError:
+        return None, None
+    m = re.search(re.escape(kernel_tag) + r".*?\n.*?(\d+) bytes spill stores, (\d+) bytes spill loads\n.*?Used (\d+) registers",
+                  log, re.S)
+    return (int(m.group(3)), int(m.group(1)) + int(m.group(2))) if m else (None, None)
+
+
 def run_ours(args, cfg, order, tangent):
     import torch
     import torch.distributed as dist
@@ -383,7 +395,8 @@ def run_ours(args, cfg, order, tangent):
     build_hash = awbuild.source_hash()
     traffic, traffic_src = (None, None) if world > 1 else measured_traffic(
         build_hash, kernel_name, args.config, int(steps_per_launch))
-    roofline = {"bound": "alu", "kernel": kernel_name,
+    regs, spill = ptxas_report("integrate_kernelILi%dELb%dELi%dE" % (3 if order == 4 else 7, int(tangent), level))
+    roofline = {"bound": "alu", "kernel": kernel_name, "registers_per_thread": regs, "spill_bytes": spill,
                 "achieved": achieved, "peak": FP64_PEAK_TFLOPS_NOMINAL, "unit": "TFLOP/s",
                 "frac": achieved / FP64_PEAK_TFLOPS_NOMINAL, "traffic": traffic, "traffic_source": traffic_src,
                 "build_hash": build_hash,
@@ -402,7 +415,7 @@ def run_ours(args, cfg, order, tangent):
                 "fp64_issue_cycles_per_step_model": mix["issue_cycles"],
                 "three_register_fp64_per_step": mix["three_register_fp64"],
                 "fp64_pipe_busy_ceiling_model": 2.0 * (mix["dfma"] + mix["dmul"] + mix["dadd"]) / mix["issue_cycles"],
-                "trig_level": level, "block_threads": aw.aw_block_size(ens),
+                "trig_level": level, "block_threads": aw.aw_block_size(ens, cfg["dt"]),
                 "launch_ms": launch_ms, "launches_timed": n_integ_launches,
                 "kernel_share_of_step": integ_ms / total_ms}
 

@@ -254,10 +254,12 @@ AW_API int aw_stage_constants(int order, double dt, double eps, double *a_host, 
  * (6,7), (7,8), 8 and 9 = mixed (rotations through the shorter drifts, device sincos after the long ones); or a
  * negative aw_status.  Pure host arithmetic. */
 AW_API int aw_trig_level(const aw_state *s, double dt);
-/* Threads per block aw_integrate launches for this state: s->block if forced, else 128 when ceil(n/128) fills every
- * SM with its 4 resident blocks, else 64 or 32 so that a small ensemble's warps spread over all SMs (queries the
- * current device's SM count; 148 if there is none).  The result of aw_integrate does not depend on it. */
-AW_API int aw_block_size(const aw_state *s);
+/* Threads per block aw_integrate launches for this state and dt: s->block if forced, else 128 when ceil(n/128) fills
+ * every SM with its 4 resident blocks, else the smallest of 32, 64, 128 whose blocks are all resident at once (16 per
+ * SM; 6 per SM for the trigonometry levels that keep the 32 KB sincos table in shared memory), so that a small
+ * ensemble's warps spread over all SMs (queries the current device's SM count; 148 if there is none).  The result
+ * of aw_integrate does not depend on it.  Negative aw_status as aw_trig_level. */
+AW_API int aw_block_size(const aw_state *s, double dt);
 /* The common tangent vector of tangent_mode 0: unit vector from u(seed, 2^63-1, 5..10) (R12). */
 AW_API int aw_common_tangent(uint64_t seed, double *t6_host);
 

@@ -104,7 +104,7 @@ def lib():
         L.aw_velocity_map_host.argtypes = [C.POINTER(AwState), C.POINTER(HostIn), i64, dbl, i64, C.c_int, i32, i32,
                                            dbl, dbl, vp, C.POINTER(HostOut)]
         L.aw_bound_energy.argtypes = [C.POINTER(AwState), vp]
-        L.aw_block_size.argtypes = [C.POINTER(AwState)]
+        L.aw_block_size.argtypes = [C.POINTER(AwState), dbl]
         _lib = L
     return _lib
 
@@ -155,8 +155,8 @@ def aw_trig_level(ens, dt):
     return _check(lib().aw_trig_level(C.byref(ens.c), dt), "aw_trig_level")
 
 
-def aw_block_size(ens):
-    return _check(lib().aw_block_size(C.byref(ens.c)), "aw_block_size")
+def aw_block_size(ens, dt):
+    return _check(lib().aw_block_size(C.byref(ens.c), dt), "aw_block_size")
 
 
 def aw_common_tangent(seed):

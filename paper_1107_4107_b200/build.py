@@ -17,7 +17,7 @@ SOURCES = ["aw_api.cu", "aw_integrate.cu", "aw_init.cu", "aw_reduce.cu"]
 UNITS = [("aw_api.cu", "aw_api.o", []), ("aw_integrate.cu", "aw_integrate.o", []),
          ("aw_integrate.cu", "aw_integrate_low.o", ["-DAW_LEVEL_GROUP=1", "-Xptxas", "-O1"]),
          ("aw_init.cu", "aw_init.o", []), ("aw_reduce.cu", "aw_reduce.o", [])]
-HEADERS = ["aw_internal.cuh", "aw_trig.cuh", "aw_trig_coeffs.h", "aw_trig_table.h", "aw_model.cuh", os.path.join("..", "..", "include", "aw.h")]
+HEADERS = ["aw_internal.cuh", "aw_trig.cuh", "aw_trig_coeffs.h", "aw_trig_table.h", "aw_tsincos.cuh", "aw_model.cuh", os.path.join("..", "..", "include", "aw.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-Xptxas", "-v"]
 

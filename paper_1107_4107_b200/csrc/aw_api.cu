@@ -258,10 +258,12 @@ int aw_trig_level(const aw_state *s, double dt) {
   return trig_level_for(amax * std::sqrt(2.0 * (energy_bound(s) + 2.0 * std::fabs(s->eps))));
 }
 
-int aw_block_size(const aw_state *s) {
+int aw_block_size(const aw_state *s, double dt) {
   if (!s || s->n < 0) return AW_EINVAL;
   if (s->block != 0 && s->block != 32 && s->block != 64 && s->block != 128) return AW_EINVAL;
-  return integrate_block_size(s->n, s->block);
+  const int level = aw_trig_level(s, dt);
+  if (level < 0) return level;
+  return integrate_block_size(s->n, s->block, kernel_uses_table(s->order, level));
 }
 
 int aw_common_tangent(uint64_t seed, double *t6_host) {
@@ -357,7 +359,7 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
     const cudaError_t e = launch_range_check(s->q, s->status, s->n, s->pitch, s->eps, hmax, (cudaStream_t)s->stream);
     if (e != cudaSuccess) return cuda_fail(e);
   }
-  p.block = integrate_block_size(s->n, s->block);
+  p.block = integrate_block_size(s->n, s->block, kernel_uses_table(s->order, p.level));
   const int64_t pieces = (stride + kMaxChunk - 1) / kMaxChunk;
   p.chunk = (int32_t)((stride + pieces - 1) / pieces);
 

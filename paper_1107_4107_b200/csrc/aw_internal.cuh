@@ -66,7 +66,8 @@ cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, 
 int trig_level_for(double max_drift_angle);
 // largest drift angle max_s |a_s| * max|p| the level supports (infinity for level 0)
 double trig_level_max_angle(int level);
-int integrate_block_size(int64_t n, int forced);
+int integrate_block_size(int64_t n, int forced, bool uses_table);
+bool kernel_uses_table(int order, int level);
 // true if |a_loop[s]| / max |a_loop| are within the ratios the per-drift Taylor degrees were derived for
 bool drift_ratios_hold(int S, const double *a_loop);
 constexpr int kMaxChunk = 128;

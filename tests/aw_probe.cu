@@ -6,6 +6,7 @@
 #include "../paper_1107_4107_b200/csrc/aw_internal.cuh"
 #include "../paper_1107_4107_b200/csrc/aw_model.cuh"
 #include "../paper_1107_4107_b200/csrc/aw_trig.cuh"
+#include "../paper_1107_4107_b200/csrc/aw_tsincos.cuh"
 #include "aw_probe.h"
 
 namespace {
@@ -24,6 +25,21 @@ __global__ void sincos_kernel(const double *x, int64_t n, double *s, double *c) 
   if (i < n) {
     double sn, cs;
     sincos(x[i], sn, cs);
+    s[i] = sn;
+    c[i] = cs;
+  }
+}
+
+__global__ void tsincos_kernel(const double *x, int64_t n, double *s, double *c) {
+  __shared__ double2 tab_s[aw::kTab * aw::kTabCopies];
+  for (int i = threadIdx.x; i < aw::kTab * aw::kTabCopies; i += blockDim.x)
+    tab_s[i] = make_double2(aw_trig_table[2 * (i / aw::kTabCopies)], aw_trig_table[2 * (i / aw::kTabCopies) + 1]);
+  __syncthreads();
+  const aw::TrigTable tab = {reinterpret_cast<const char *>(tab_s), (threadIdx.x & (aw::kTabCopies - 1)) * 16u};
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) {
+    double sn, cs;
+    aw::tsincos(tab, x[i], sn, cs);
     s[i] = sn;
     c[i] = cs;
   }
@@ -148,6 +164,14 @@ int awp_sincos(const double *x_dev, int64_t n, double *sin_dev, double *cos_dev,
   if (n == 0) return 0;
   cudaStream_t st = (cudaStream_t)stream;
   sincos_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(x_dev, n, sin_dev, cos_dev);
+  return done(st);
+}
+
+int awp_tsincos(const double *x_dev, int64_t n, double *sin_dev, double *cos_dev, void *stream) {
+  if (!x_dev || !sin_dev || !cos_dev || n < 0) return -1;
+  if (n == 0) return 0;
+  cudaStream_t st = (cudaStream_t)stream;
+  tsincos_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(x_dev, n, sin_dev, cos_dev);
   return done(st);
 }
 

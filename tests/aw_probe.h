@@ -20,6 +20,8 @@ extern "C" {
 
 /* Device sincos used by the integrator (csrc/aw_trig.cuh, pin P14), on n device doubles. */
 AWP_API int awp_sincos(const double *x_dev, int64_t n, double *sin_dev, double *cos_dev, void *stream);
+/* Table-driven sincos of the step loop (csrc/aw_tsincos.cuh; DESIGN.md §6.1 (ii)), on n device doubles, |x| < 1024. */
+AWP_API int awp_tsincos(const double *x_dev, int64_t n, double *sin_dev, double *cos_dev, void *stream);
 /* u(seed, k0 + i, slot) for i in [0, n) written to out_dev (device); include/aw.h, R11. */
 AWP_API int awp_uniform(uint64_t seed, uint64_t k0, int64_t n, uint32_t slot, double *out_dev, void *stream);
 /* H(X,P) by the device routine the checkpoint uses, for n states in SoA planes q (6*pitch). */

@@ -15,7 +15,8 @@ _SRC = os.path.join(_HERE, "aw_probe.cu")
 _LIB = os.path.join(_HERE, "libaw_probe.so")
 _CSRC = os.path.join(os.path.dirname(_HERE), "paper_1107_4107_b200", "csrc")
 _DEPS = [_SRC, os.path.join(_HERE, "aw_probe.h")] + [os.path.join(_CSRC, f) for f in
-                                                    ("aw_internal.cuh", "aw_trig.cuh", "aw_trig_coeffs.h", "aw_model.cuh")]
+                                                    ("aw_internal.cuh", "aw_trig.cuh", "aw_trig_coeffs.h", "aw_model.cuh",
+                                                     "aw_tsincos.cuh", "aw_trig_table.h")]
 _lib = None
 
 
@@ -40,6 +41,7 @@ def lib():
         L = C.CDLL(build())
         vp, i64, dbl, u64 = C.c_void_p, C.c_int64, C.c_double, C.c_uint64
         L.awp_sincos.argtypes = [vp, i64, vp, vp, vp]
+        L.awp_tsincos.argtypes = [vp, i64, vp, vp, vp]
         L.awp_uniform.argtypes = [u64, u64, i64, C.c_uint32, vp, vp]
         L.awp_hamiltonian.argtypes = [vp, i64, i64, dbl, vp, vp]
         L.awp_dfma_peak.argtypes = [C.c_int, C.c_int, C.c_int, i64, vp, C.POINTER(dbl), C.POINTER(dbl), vp]
@@ -63,6 +65,15 @@ def sincos(x):
     s, c = torch.empty_like(x), torch.empty_like(x)
     _ok(lib().awp_sincos(C.c_void_p(x.data_ptr()), x.numel(), C.c_void_p(s.data_ptr()), C.c_void_p(c.data_ptr()),
                          _stream()), "awp_sincos")
+    return s, c
+
+
+def tsincos(x):
+    """The table-driven sincos of the integrator's step loop (csrc/aw_tsincos.cuh)."""
+    import torch
+    s, c = torch.empty_like(x), torch.empty_like(x)
+    _ok(lib().awp_tsincos(C.c_void_p(x.data_ptr()), x.numel(), C.c_void_p(s.data_ptr()), C.c_void_p(c.data_ptr()),
+                          _stream()), "awp_tsincos")
     return s, c
 
 

@@ -41,7 +41,7 @@ def test_probe_library_exports_its_header():
     import aw_probe
     src = open(os.path.join(ROOT, "tests", "aw_probe.h")).read()
     names = sorted(set(re.findall(r"AWP_API\s+[\w\s\*]+?\b(awp_\w+)\s*\(", src)))
-    assert names == ["awp_dfma_peak", "awp_dfma_shape", "awp_hamiltonian", "awp_sincos", "awp_uniform"]
+    assert names == ["awp_dfma_peak", "awp_dfma_shape", "awp_hamiltonian", "awp_sincos", "awp_tsincos", "awp_uniform"]
     L = C.CDLL(aw_probe.build())
     for n in names:
         assert hasattr(L, n), n

@@ -34,6 +34,51 @@ def aw():
     return aw
 
 
+# ------------------------------------------------------------------ table-driven sincos of the step loop
+
+def test_table_sincos_within_2ulp(aw):
+    """csrc/aw_tsincos.cuh (DESIGN.md §6.1 (ii)) against libm / mpmath on 5e6 random points of the range the integrator
+    produces (|x| < 1024, R7), every table grid point and the midpoints between them: <= 2 ulp of max(|result|, s1)
+    with s1 = sin(2 pi / 512) = 0.0123 — the statement pin P14 makes for the device sincos wherever |result| >= s1, and
+    an absolute 3.5e-18 nearer a zero of the function, where the result is the difference of a table entry and a
+    correction of the same size (the kick multiplies it by O(1) factors: what matters there is the error relative to
+    the amplitude, 0.016 ulp).  Exact at 0, sin bit-odd and cos bit-even."""
+    import aw_probe
+    rng = np.random.default_rng(41)
+    grid = np.arange(-2048, 2049) * (2 * math.pi / 512)
+    x = np.concatenate([rng.uniform(-16 * math.pi, 16 * math.pi, 4_000_000), rng.uniform(-1024.0, 1024.0, 1_000_000),
+                        rng.uniform(-1e-3, 1e-3, 100_000), grid, grid + math.pi / 512,
+                        np.array([0.0, -0.0, math.pi, -math.pi, math.pi / 2, 1e-300, 5e-324])])
+    s, c = aw_probe.tsincos(torch.from_numpy(x).cuda())
+    s, c = s.cpu().numpy(), c.cpu().numpy()
+    rs, rc = np.sin(x), np.cos(x)
+
+    s1 = math.sin(2 * math.pi / 512)
+    floor_ulp = np.spacing(s1)
+
+    def excess(a, b):
+        return np.abs(a - b) - 2.0 * np.maximum(np.spacing(np.abs(b)), floor_ulp)
+    assert excess(s, rs).max() <= 0.0, excess(s, rs).max()
+    assert excess(c, rc).max() <= 0.0, excess(c, rc).max()
+    nr = 5_100_000
+    ulps = lambda a, b: np.abs(a - b) / np.maximum(np.spacing(np.abs(b)), floor_ulp)
+    assert ulps(s[:nr], rs[:nr]).max() <= 2.0 and ulps(c[:nr], rc[:nr]).max() <= 2.0
+    import mpmath as mp
+    mp.mp.dps = 40
+    for i in rng.integers(0, nr, 2000):
+        xs = mp.mpf(float(x[i]))
+        es = abs(mp.mpf(float(s[i])) - mp.sin(xs)) / mp.mpf(float(max(np.spacing(abs(rs[i])), floor_ulp)))
+        ec = abs(mp.mpf(float(c[i])) - mp.cos(xs)) / mp.mpf(float(max(np.spacing(abs(rc[i])), floor_ulp)))
+        assert es <= 1.6 and ec <= 1.6, (x[i], es, ec)
+    s0, c0 = aw_probe.tsincos(torch.zeros(1, dtype=torch.float64, device="cuda"))
+    assert s0.item() == 0.0 and c0.item() == 1.0
+    sm, cm = aw_probe.tsincos(torch.from_numpy(-x).cuda())
+    assert np.array_equal(sm.cpu().numpy(), -s) and np.array_equal(cm.cpu().numpy(), c)
+    # agreement with the device sincos the checkpoints use: both within 2 ulp of the truth
+    sd, cd = aw_probe.sincos(torch.from_numpy(x[:nr]).cuda())
+    assert ulps(s[:nr], sd.cpu().numpy()).max() <= 4.0 and ulps(c[:nr], cd.cpu().numpy()).max() <= 4.0
+
+
 # ------------------------------------------------------------------ P:97 Gaussian cloud (shape 2)
 
 @pytest.mark.parametrize("E,eps,cx,cy,sigma,pz_sign", [
