@@ -171,21 +171,23 @@ AW_API int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps,
  * backwards).  steps == 0 or n == 0 is a no-op.  AW_ERANGE if stride*|dt|*sqrt(2(E+2|eps|)) >= 1024
  * (the angle would leave the range the two-constant argument reduction handles exactly, R7).
  * AW_ESTATE if !s->ready or order not in {4, 6}.  Advances s->t and s->step.
- * Trigonometry: the kick needs sin/cos of x, y and 2z at every stage.  With s->trig == 0 the kernel
- * carries the three (sin, cos) pairs (of x + y, x - y and 2z) in registers and advances them through each drift by a rotation
- * with the drift angle d = a_s p (Taylor polynomials in d; the degree is picked on the host from
- * max_s |a_s| sqrt(2(E + 2|eps|)) so the truncation stays below 2^-60; aw_trig_level reports it), and
- * recomputes them from the angles with the device sincos at every checkpoint and at least every 128
- * steps.  The bound is max(s->E, s->Emax) and it is ENFORCED: every call first runs one elementwise kernel that
+ * Trigonometry: the kick needs sin/cos of x + y, x - y and 2z at every stage.  With s->trig == 0 the kernel carries
+ * the three (sin, cos) pairs in registers and advances a pair through a drift by a rotation with the drift angle
+ * d = A p (Taylor polynomials in p with the powers of A folded into the coefficients) whenever degree <= 5 keeps the
+ * truncation below 2^-60; the degree of every drift and pair type is fixed at compile time from the level the host
+ * picks (max_s |a_s| sqrt(2(Emax + 2|eps|)); aw_trig_level reports it) and the drift's ratio to the longest one.  A
+ * pair every drift rotates is recomputed from the tracked angle with the device sincos at every checkpoint and at
+ * least every 128 steps.  After a drift too long to rotate through, the kick evaluates the pair from the angle with
+ * a table-driven sincos (512-entry table of the whole circle in shared memory + degree-2 residual rotation; no
+ * quadrant logic); from level 5 on the kernels mix the two per drift and per pair, and at level 0 (drift angle
+ * beyond 2 rad, or s->trig == 1) every stage uses the table.
+ * The bound is max(s->E, s->Emax) and it is ENFORCED: every call first runs one elementwise kernel that
  * evaluates each live trajectory's H(X,P) and compares it with the largest energy the chosen level (and the angle
  * range of R7) supports; above it the trajectory gets AW_ST_RANGE and is not touched (P^2 <= 2(H + 2|eps|)
  * along the whole orbit, so the check before the first step covers every step).  The flag is a status like any other:
  * to integrate such a trajectory after all, set its status byte back to AW_ST_LIVE and raise the bound (aw_bound_energy
- * considers live trajectories only).  Call aw_bound_energy after uploading a state whose
- * energy the struct does not know.  If the drift angle can exceed
- * 0.357 rad the kernel is mixed (levels 8 and 9, up to 0.54 and 2 rad): the scheme's shorter drifts still rotate the
- * pairs, the long ones are followed by the device sincos; beyond 2 rad, or with s->trig == 1, the device sincos is evaluated at
- * every stage (level 0).
+ * considers live trajectories only).  Call aw_bound_energy after uploading a state whose energy the struct does not
+ * know.
  * The work is split into kernel launches of at most AW_MAX_STEPS_PER_LAUNCH steps (a multiple of
  * stride); the result does not depend on the split. */
 #define AW_MAX_STEPS_PER_LAUNCH 20000
@@ -249,10 +251,10 @@ AW_API int aw_bound_energy(aw_state *s, void *scratch_dev);
  * order 6) or AW_EINVAL.  Order-6 weights are obtained inside the library by Newton iteration on the
  * four order conditions in extended precision. */
 AW_API int aw_stage_constants(int order, double dt, double eps, double *a_host, double *b_host);
-/* Trigonometry level aw_integrate would use for this state and dt: 0 = device sincos at every stage,
- * 1..7 = running pairs with Taylor degrees (x+y / x-y pairs, 2z pair) = (3,3), (3,4), (4,4), (4,5), (5,6),
- * (6,7), (7,8), 8 and 9 = mixed (rotations through the shorter drifts, device sincos after the long ones); or a
- * negative aw_status.  Pure host arithmetic. */
+/* Trigonometry level aw_integrate would use for this state and dt: the bracket of the largest drift angle
+ * d = max_s |a_s| sqrt(2(max(E, Emax) + 2|eps|)): 1..9 <-> d <= 0.0104, 0.0147, 0.0354, 0.05, 0.1166, 0.2192, 0.357,
+ * 0.54, 2; 0 = beyond (or s->trig == 1): table-driven sincos at every stage.  Levels 1-4 rotate every pair through
+ * every drift; from level 5 on the long drifts go through the table; or a negative aw_status.  Pure host arithmetic. */
 AW_API int aw_trig_level(const aw_state *s, double dt);
 /* Threads per block aw_integrate launches for this state and dt: s->block if forced, else 128 when ceil(n/128) fills
  * every SM with its 4 resident blocks, else the smallest of 32, 64, 128 whose blocks are all resident at once (16 per

@@ -116,7 +116,7 @@ __device__ __forceinline__ void rotate(double &s, double &c, double g, double m)
 // 1..7; the short inner drifts of the triple jump (ratio 0.13) and of the 7-stage scheme (0.088) one or two less.
 // A drift whose own largest angle needs more than degree kMaxRotDegree leaves that pair type stale, and the kick that
 // follows evaluates the table-driven sincos instead (degree 0 below); the decision is per drift and per pair type, so
-// from level 4 on the kernels are mixed: the short inner drifts rotate, the long ones (first the zeta pair, which
+// from level 5 on the kernels are mixed: the short inner drifts rotate, the long ones (first the zeta pair, which
 // turns sqrt(2) faster) go through tsincos.  A pair type with a stale drift is recomputed in every step and needs no
 // re-synchronisation.
 constexpr double kLevelMaxD[10] = {0.0, 0.0104, 0.0147, 0.0354, 0.0500, 0.1166, 0.2192, 0.3570, 0.5400, 2.0};

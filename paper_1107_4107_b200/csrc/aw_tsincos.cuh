@@ -5,7 +5,7 @@
 
 namespace aw {
 
-// Table-driven sincos for the kicks that follow a drift too long to rotate through (from level 4 on, and at every
+// Table-driven sincos for the kicks that follow a drift too long to rotate through (from level 5 on, and at every
 // stage of level 0): the angle is split as x = k (2 pi / T) + r, |r| <= pi / T, the pair of the grid point k mod T comes
 // from a table of T = 256 correctly rounded (sin, cos) values in shared memory (csrc/aw_trig_table.h, whole circle),
 // and is rotated by the residual r with the same short Taylor series as the drift rotations (|r| <= 0.0123: sin to

@@ -167,6 +167,21 @@ def test_validation_happens_on_the_host(aw):
     st.block = 48
     assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == EINVAL
     st.block = 0
+    # aw_block_size: the smallest block whose grid is resident at once (16 blocks per SM; 6 for the trigonometry levels
+    # that hold the 32 KB table in shared memory), 128 once that fills the chip (148 SMs assumed without a device)
+    L.aw_block_size.argtypes = [C.POINTER(AwState), C.c_double]
+    bs = AwState(); bs.E, bs.eps, bs.order = 1.0, 3e-2, 4
+    def block(n, dt, order=4, E=1.0, eps=3e-2):
+        bs.n, bs.order, bs.E, bs.eps = n, order, E, eps
+        return L.aw_block_size(C.byref(bs), dt)
+    assert [block(n, 0.005) for n in (1, 4096, 32000, 75648, 75649, 1 << 22)] == [32, 32, 32, 32, 128, 128]
+    assert lv(0.005) == 1 and block(32000, 0.2) == 64            # level 8: table kernel, 1000 blocks of 32 > 148 x 6
+    assert block(28000, 0.2) == 32 and block(57000, 0.2) == 128   # 875 blocks fit; 891 blocks of 64 do not
+    assert block(32000, 0.0628, order=6, E=15.0, eps=1.0) == 64   # the paper's Fig. 4 ensemble
+    bs.block = 128
+    assert block(5, 0.005) == 128
+    bs.block = 0
+    assert block(5, 0.0) == EINVAL
     # Emax raises the energy bound the trig level (and the R7 range) is sized for; below E it is ignored
     st.Emax = 0.0
     assert lv(0.005) == 1

@@ -381,6 +381,34 @@ def test_slices_are_bit_identical_to_the_whole(aw, orc, shape, angle_mode, tmode
         aw.aw_init_shell(aw.Ensemble(5, tangent=False, wind=False), mk(aw, n - 4), E, eps, seed)
 
 
+# ------------------------------------------------------------------ negative perturbation strength
+
+@pytest.mark.parametrize("order,dt", [(4, 0.005), (6, 0.02), (4, 0.1), (6, 0.4)])
+def test_negative_eps_parity(aw, orc, order, dt):
+    """eps < 0 is a legal model (E - 2|eps| > 0): every stage weight b_s changes sign, and with it the factor 2 b_0 the
+    kernel scales its carried zeta pair by.  Rotation and table kernels, tangent map on."""
+    gx, gy = 67, 33
+    n = gx * gy
+    ens = aw.Ensemble(n, tangent=True, wind=True, order=order)
+    aw.aw_init_shell(ens, aw.make_grid(gx, gy, -1.0, 1.0, angle_mode=1), 1.0, -3e-2, 13)
+    st = ensemble_to_oracle(ens, orc)
+    steps = 1000 if dt < 0.1 else 200
+    aw.aw_integrate(ens, n, steps, dt, 100)
+    oracle_integrate_mt(orc, st, steps, dt, 100)
+    got = ensemble_to_oracle(ens, orc)
+    assert np.array_equal(got.status, st.status)
+    live = st.status == 1
+    thr = math.log(st.t) + 3.0
+    regular = live & (st.acc[1, :n] <= thr)
+    assert regular.sum() > 0.5 * live.sum()
+    err = state_rel_err(got.q[:, :n], got.wind[:, :n], st.q[:, :n], st.wind[:, :n], regular)
+    assert err.max() <= 1e-10, err.max()
+    lo10 = live & (st.acc[1, :n] < 10)
+    assert np.max(np.abs(got.acc[1, :n][lo10] - st.acc[1, :n][lo10])) <= 1e-5
+    P2 = (got.q[3:, :n][:, live] ** 2).sum(0)
+    assert np.all(np.abs(P2 - 2.0) <= 4 * 3e-2 + 1e-6)                     # shell layer, P:51
+
+
 # ------------------------------------------------------------------ block size
 
 @pytest.mark.parametrize("order,tangent,dt", [(4, True, 0.005), (6, False, 0.0628), (6, True, 0.3), (4, False, 1.2)])
