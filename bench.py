@@ -382,7 +382,8 @@ def run_ours(args, cfg, order, tangent):
     max_launch = 20000 // cfg["stride"] * cfg["stride"]                  # AW_MAX_STEPS_PER_LAUNCH (include/aw.h)
     n_integ_launches = args.steps * sum(math.ceil(c / max_launch) for c in calls)
     level = aw.aw_trig_level(ens, cfg["dt"])
-    mix = sass_count.integrate_step_mix(order, tangent, level)
+    schedule = aw.aw_kernel_schedule(ens, cfg["dt"])      # 1: throughput flavour, 0: latency flavour (small ensembles)
+    mix = sass_count.integrate_step_mix(order, tangent, level, schedule=schedule)
     flops_nominal = NOMINAL_FLOPS[(order, tangent)]
     flops_per_step = min(flops_nominal, mix["flops"])
     launch_ms = integ_ms / n_integ_launches
@@ -391,11 +392,12 @@ def run_ours(args, cfg, order, tangent):
     achieved = kernel_rate * flops_per_step / 1e12
     sms = torch.cuda.get_device_properties(dev).multi_processor_count
     fp64_slots = sms * 64 * 1.965e9                                      # fp64 thread-instructions / s
-    kernel_name = "integrate_kernel<%d,%s,%d>" % (3 if order == 4 else 7, str(tangent).lower(), level)
+    kernel_name = "integrate_kernel<%d,%s,%d,%d>" % (3 if order == 4 else 7, str(tangent).lower(), level, schedule)
     build_hash = awbuild.source_hash()
     traffic, traffic_src = (None, None) if world > 1 else measured_traffic(
         build_hash, kernel_name, args.config, int(steps_per_launch))
-    regs, spill = ptxas_report("integrate_kernelILi%dELb%dELi%dE" % (3 if order == 4 else 7, int(tangent), level))
+    regs, spill = ptxas_report("integrate_kernelILi%dELb%dELi%dELi%dE" % (3 if order == 4 else 7, int(tangent), level,
+                                                                          schedule))
     roofline = {"bound": "alu", "kernel": kernel_name, "registers_per_thread": regs, "spill_bytes": spill,
                 "achieved": achieved, "peak": FP64_PEAK_TFLOPS_NOMINAL, "unit": "TFLOP/s",
                 "frac": achieved / FP64_PEAK_TFLOPS_NOMINAL, "traffic": traffic, "traffic_source": traffic_src,

@@ -105,7 +105,10 @@ typedef struct {
                       from the data (uploaded states); 0 / NaN = use E                              */
   int32_t block;   /* threads per block of the integrator: 0 (default) = chosen from n so that small ensembles
                       spread over all SMs; 32, 64 or 128 = forced.  The result does not depend on it    */
-  int32_t reserved_;
+  int32_t flavour; /* the integrator kernels exist in two ptxas schedules of the same source and arithmetic: 1 = scheduled
+                      for throughput (operand reuse; best with >= 3 warps per sub-partition), 2 = for latency
+                      (interleaved chains; best for small ensembles); 0 (default) = chosen from n (latency up to
+                      151 552 trajectories on a B200).  The result does not depend on it                 */
 } aw_state;
 
 /* Initial-condition family (P:85 whole region, P:87 patch, P:97 cloud; R6, R8, R9, R12, R17, R18). */
@@ -262,6 +265,10 @@ AW_API int aw_trig_level(const aw_state *s, double dt);
  * ensemble's warps spread over all SMs (queries the current device's SM count; 148 if there is none).  The result
  * of aw_integrate does not depend on it.  Negative aw_status as aw_trig_level. */
 AW_API int aw_block_size(const aw_state *s, double dt);
+/* Which ptxas schedule of the integrator kernel aw_integrate launches for this state and dt (aw_state.flavour): 1 = the
+ * throughput flavour, 0 = the latency flavour (always 0 for the levels that exist in one flavour only: 0, 8, 9); or a
+ * negative aw_status.  The kernel is integrate_kernel<S, TAN, LEVEL, SCHEDULE> with S = 3 / 7 stages. */
+AW_API int aw_kernel_schedule(const aw_state *s, double dt);
 /* The common tangent vector of tangent_mode 0: unit vector from u(seed, 2^63-1, 5..10) (R12). */
 AW_API int aw_common_tangent(uint64_t seed, double *t6_host);
 

@@ -39,7 +39,7 @@ class AwState(C.Structure):
                 ("qref", C.c_void_p), ("windref", C.c_void_p), ("tref", C.c_double),
                 ("surv_lo_x", C.c_double), ("surv_hi_x", C.c_double),
                 ("surv_lo_y", C.c_double), ("surv_hi_y", C.c_double),
-                ("Emax", C.c_double), ("block", C.c_int32), ("reserved_", C.c_int32)]
+                ("Emax", C.c_double), ("block", C.c_int32), ("flavour", C.c_int32)]
 
 
 class Grid(C.Structure):
@@ -105,6 +105,7 @@ def lib():
                                            dbl, dbl, vp, C.POINTER(HostOut)]
         L.aw_bound_energy.argtypes = [C.POINTER(AwState), vp]
         L.aw_block_size.argtypes = [C.POINTER(AwState), dbl]
+        L.aw_kernel_schedule.argtypes = [C.POINTER(AwState), dbl]
         _lib = L
     return _lib
 
@@ -157,6 +158,10 @@ def aw_trig_level(ens, dt):
 
 def aw_block_size(ens, dt):
     return _check(lib().aw_block_size(C.byref(ens.c), dt), "aw_block_size")
+
+
+def aw_kernel_schedule(ens, dt):
+    return _check(lib().aw_kernel_schedule(C.byref(ens.c), dt), "aw_kernel_schedule")
 
 
 def aw_common_tangent(seed):
@@ -221,6 +226,14 @@ class Ensemble:
     @block.setter
     def block(self, v):
         self.c.block = v
+
+    @property
+    def flavour(self):
+        return self.c.flavour
+
+    @flavour.setter
+    def flavour(self, v):
+        self.c.flavour = v
 
     @property
     def trig(self):

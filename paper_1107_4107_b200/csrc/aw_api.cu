@@ -203,6 +203,7 @@ static int validate_integrate_args(const aw_state *s, int64_t steps, double dt, 
   if (s->survive != 0 && s->survive != 1) return AW_EINVAL;
   if (s->survive && !(s->surv_hi_x > s->surv_lo_x && s->surv_hi_y > s->surv_lo_y)) return AW_EINVAL;
   if (s->block != 0 && s->block != 32 && s->block != 64 && s->block != 128) return AW_EINVAL;
+  if (s->flavour < 0 || s->flavour > 2) return AW_EINVAL;
   return AW_OK;
 }
 
@@ -264,6 +265,13 @@ int aw_block_size(const aw_state *s, double dt) {
   const int level = aw_trig_level(s, dt);
   if (level < 0) return level;
   return integrate_block_size(s->n, s->block, kernel_uses_table(s->order, level));
+}
+
+int aw_kernel_schedule(const aw_state *s, double dt) {
+  if (!s || s->n < 0 || s->flavour < 0 || s->flavour > 2) return AW_EINVAL;
+  const int level = aw_trig_level(s, dt);
+  if (level < 0) return level;
+  return (level >= 1 && level <= 7 && !integrate_latency_flavour(s->n, s->flavour)) ? 1 : 0;
 }
 
 int aw_common_tangent(uint64_t seed, double *t6_host) {
@@ -360,6 +368,7 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
     if (e != cudaSuccess) return cuda_fail(e);
   }
   p.block = integrate_block_size(s->n, s->block, kernel_uses_table(s->order, p.level));
+  const bool latency = integrate_latency_flavour(s->n, s->flavour);
   const int64_t pieces = (stride + kMaxChunk - 1) / kMaxChunk;
   p.chunk = (int32_t)((stride + pieces - 1) / pieces);
 
@@ -371,7 +380,7 @@ int aw_integrate(aw_state *s, int64_t n, int64_t steps, double dt, int64_t strid
   for (int64_t done = 0; done < total_chk; done += chk_per_launch) {
     const int64_t now = (total_chk - done < chk_per_launch) ? total_chk - done : chk_per_launch;
     p.nchk = (int32_t)now;
-    const cudaError_t e = launch_integrate(p, s->order, s->w != nullptr, (cudaStream_t)s->stream);
+    const cudaError_t e = launch_integrate(p, s->order, s->w != nullptr, latency, (cudaStream_t)s->stream);
     if (e != cudaSuccess) return cuda_fail(e);
     s->step = step0 + (done + now) * stride;
     s->t = t0 + (double)(s->step - step0) * std::fabs(dt);

@@ -52,13 +52,19 @@
 #define AW_MIN_BLOCKS(LEVEL) ((LEVEL) == 4 ? 4 : 3)
 #endif
 
-// This file is compiled twice (build.py).  AW_LEVEL_GROUP 1 instantiates the rotation kernels (trig levels 1-7)
-// and is compiled with -Xptxas -O1: ptxas's lighter scheduler stays close to source order, which keeps the
-// three-register FMAs that share an operand next to each other, so more of them hit the operand-reuse cache
-// (measured on B200: configs[3] +3.5 %, configs[2] +3.5 %, order 6 +2.9 %, configs[4] +1.5 %, level 7 +1.6 %), and
-// needs fewer registers (the 7-stage scheme's four coefficient sets fit).  AW_LEVEL_GROUP 0 (default flags) holds
-// the kernels that evaluate the device sincos in the step loop (level 0: at every stage; the mixed levels 8, 9), which
-// lose 2-3 % at -O1, and the host-side functions.
+// This file is compiled twice (build.py), the same source and the same arithmetic under two ptxas schedules:
+//   AW_LEVEL_GROUP 1, -Xptxas -O1, trig levels 1-7: the lighter scheduler stays close to source order, which keeps the
+//     three-register FMAs that share an operand next to each other, so more of them hit the operand-reuse cache
+//     (measured on B200: configs[3] +3.5 %, configs[2] +3.5 %, order 6 +2.9 %), and needs fewer registers.  This is
+//     the THROUGHPUT flavour: best when the fp64 pipe is saturated (>= 3 warps per sub-partition).
+//   AW_LEVEL_GROUP 0, default flags, every level: ptxas interleaves the independent chains of a stage (the three pairs'
+//     polynomials, the three table look-ups), which is what a warp needs when it has a sub-partition almost to itself.
+//     This is the LATENCY flavour, used for small ensembles (the paper's Fig. 4 ensemble, 32 000 trajectories = 1.7
+//     warps per sub-partition: 2.94e10 -> 3.56e10 traj-steps/s; configs[0], 4096 trajectories: 1.46e10 -> 2.28e10;
+//     the same kernels on 6e5 trajectories: -1 to -3 %), and the
+//     only one for the levels whose step loop is dominated by the table sincos (0, 8, 9: -3 % at -O1).  It also holds
+//     the host-side functions.
+// ptxas does not reassociate floating-point arithmetic, so both flavours give the same bits (tested).
 #ifndef AW_LEVEL_GROUP
 #define AW_LEVEL_GROUP 0
 #endif
@@ -332,7 +338,9 @@ __device__ __forceinline__ void stages(Traj<TAN> &t, const IntegrateParams &p, c
   }
 }
 
-template <int S, bool TAN, int LEVEL>
+// SCHEDULE = AW_LEVEL_GROUP: 1 = the throughput flavour (-Xptxas -O1 unit), 0 = the latency flavour (default flags).  It
+// changes nothing in the code; it only gives the two compilations of the same kernel different names.
+template <int S, bool TAN, int LEVEL, int SCHEDULE>
 __global__ void __launch_bounds__(AW_BLOCK, AW_MIN_BLOCKS(LEVEL))
     integrate_kernel(const __grid_constant__ IntegrateParams p) {
   // the (sin, cos) table of tsincos, 4 interleaved copies, 32 KB of shared memory (kernels with a stale drift only)
@@ -424,7 +432,7 @@ template <int S, bool TAN, int LEVEL>
 cudaError_t launch_one(const IntegrateParams &p, cudaStream_t st) {
   const int block = p.block;
   const int64_t blocks = (p.n + block - 1) / block;
-  integrate_kernel<S, TAN, LEVEL><<<(unsigned)blocks, block, 0, st>>>(p);
+  integrate_kernel<S, TAN, LEVEL, AW_LEVEL_GROUP><<<(unsigned)blocks, block, 0, st>>>(p);
   count_launch();
   return cudaGetLastError();
 }
@@ -442,6 +450,13 @@ cudaError_t launch_level(const IntegrateParams &p, cudaStream_t st) {
     case 7: return launch_one<S, TAN, 7>(p, st);
     default: return cudaErrorInvalidValue;
 #else
+    case 1: return launch_one<S, TAN, 1>(p, st);
+    case 2: return launch_one<S, TAN, 2>(p, st);
+    case 3: return launch_one<S, TAN, 3>(p, st);
+    case 4: return launch_one<S, TAN, 4>(p, st);
+    case 5: return launch_one<S, TAN, 5>(p, st);
+    case 6: return launch_one<S, TAN, 6>(p, st);
+    case 7: return launch_one<S, TAN, 7>(p, st);
     case 8: return launch_one<S, TAN, 8>(p, st);
     case 9: return launch_one<S, TAN, 9>(p, st);
     default: return launch_one<S, TAN, 0>(p, st);
@@ -514,6 +529,20 @@ int integrate_block_size(int64_t n, int forced, bool uses_table) {
   return 128;
 }
 
+// Throughput or latency flavour (see AW_LEVEL_GROUP above).  Measured on B200 (latency / throughput flavour, four kernels:
+// order 4 and 6, with and without tangent, levels 1, 3, 7): x 1.4-1.9 below one warp per sub-partition (n <= 16 000),
+// x 1.0-1.2 at 1.7-5 warps, x 1.00-1.05 at 8 warps (n = 150 000), x 0.97-0.99 at 32 warps (n = 600 000): latency up
+// to 8 warps per sub-partition on average (n <= 8 x 4 x SMs x 32 = 151 552 trajectories on a B200).
+bool integrate_latency_flavour(int64_t n, int forced) {
+  if (forced == 1) return false;
+  if (forced == 2) return true;
+  int dev = 0, v = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      v <= 0)
+    v = 148;
+  return (n + 31) / 32 <= (int64_t)v * 32;
+}
+
 // The per-drift degrees assume the ratios |a_loop[cs]| / max |a_loop| of the two built-in stage lists.
 bool drift_ratios_hold(int S, const double *a_loop) {
   double amax = 0.0;
@@ -527,8 +556,8 @@ bool drift_ratios_hold(int S, const double *a_loop) {
 
 cudaError_t launch_integrate_low(const IntegrateParams &p, int order, bool tangent, cudaStream_t st);
 
-cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, cudaStream_t st) {
-  if (p.level >= 1 && p.level <= 7) return launch_integrate_low(p, order, tangent, st);
+cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, bool latency, cudaStream_t st) {
+  if (p.level >= 1 && p.level <= 7 && !latency) return launch_integrate_low(p, order, tangent, st);
   if (order == 4) return tangent ? launch_level<3, true>(p, st) : launch_level<3, false>(p, st);
   return tangent ? launch_level<7, true>(p, st) : launch_level<7, false>(p, st);
 }

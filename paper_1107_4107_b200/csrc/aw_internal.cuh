@@ -61,7 +61,9 @@ struct InitParams {
 };
 
 // host-side launchers (each returns cudaError_t of the launch and bumps the launch counter)
-cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, cudaStream_t st);
+cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, bool latency, cudaStream_t st);
+// which of the two ptxas schedules of the same kernel to launch (aw_state.flavour; aw_integrate.cu)
+bool integrate_latency_flavour(int64_t n, int forced);
 // Trigonometry variant for a largest drift angle max_s |a_s| * max|p| (0 = full sincos every stage).
 int trig_level_for(double max_drift_angle);
 // largest drift angle max_s |a_s| * max|p| the level supports (infinity for level 0)

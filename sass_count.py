@@ -26,12 +26,15 @@ def _functions(lib):
         yield chunk.split("\n", 1)[0].strip(), chunk
 
 
-def integrate_step_mix(order, tangent, level, lib=LIB):
-    """{'dfma', 'dmul', 'dadd', 'other', 'flops'} per trajectory-step of integrate_kernel<S,TAN,LEVEL>."""
-    key = (os.path.getmtime(lib), order, bool(tangent), level)
+def integrate_step_mix(order, tangent, level, lib=LIB, schedule=None):
+    """{'dfma', 'dmul', 'dadd', 'other', 'flops'} per trajectory-step of integrate_kernel<S,TAN,LEVEL,SCHEDULE>.
+    schedule: 1 = the throughput flavour (levels 1-7 only), 0 = the latency flavour; None = 1 where it exists."""
+    if schedule is None:
+        schedule = 1 if 1 <= level <= 7 else 0
+    key = (os.path.getmtime(lib), order, bool(tangent), level, schedule)
     if key in _cache:
         return _cache[key]
-    tag = "integrate_kernelILi%dELb%dELi%dE" % (3 if order == 4 else 7, 1 if tangent else 0, level)
+    tag = "integrate_kernelILi%dELb%dELi%dELi%dE" % (3 if order == 4 else 7, 1 if tangent else 0, level, schedule)
     for name, text in _functions(lib):
         if tag not in name:
             continue
@@ -85,4 +88,6 @@ if __name__ == "__main__":
     for order in (4, 6):
         for tangent in (False, True):
             for level in range(10):
-                print(order, tangent, level, integrate_step_mix(order, tangent, level))
+                for schedule in ((1, 0) if 1 <= level <= 7 else (0,)):
+                    print(order, tangent, level, "throughput" if schedule else "latency   ",
+                          integrate_step_mix(order, tangent, level, schedule=schedule))

@@ -167,6 +167,9 @@ def test_validation_happens_on_the_host(aw):
     st.block = 48
     assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == EINVAL
     st.block = 0
+    st.flavour = 3                                                         # 0 auto, 1 throughput, 2 latency
+    assert L.aw_integrate(C.byref(st), 64, 100, 0.01, 100) == EINVAL
+    st.flavour = 0
     # aw_block_size: the smallest block whose grid is resident at once (16 blocks per SM; 6 for the trigonometry levels
     # that hold the 32 KB table in shared memory), 128 once that fills the chip (148 SMs assumed without a device)
     L.aw_block_size.argtypes = [C.POINTER(AwState), C.c_double]

@@ -435,6 +435,30 @@ def test_block_size_does_not_change_the_result(aw, order, tangent, dt):
         aw.aw_integrate(bad, 64, 100, 0.01, 100)
 
 
+@pytest.mark.parametrize("order,tangent,dt", [(4, True, 0.005), (4, True, 0.025), (6, True, 0.02), (6, False, 0.0628),
+                                              (4, False, 0.1), (6, True, 0.15)])
+def test_kernel_flavours_give_the_same_bits(aw, order, tangent, dt):
+    """Trig levels 1-7 exist in two ptxas schedules of the same source (throughput: source order for operand reuse;
+    latency: interleaved chains for small ensembles); aw_integrate picks one from n.  Same arithmetic, same bits."""
+    n = 3000 + 11
+    res = []
+    for flavour in (0, 1, 2):
+        ens = aw.Ensemble(n, tangent=tangent, wind=True, order=order)
+        aw.aw_init_shell(ens, aw.make_grid(n, 1, -0.9, 0.9, angle_mode=1, lo_y=-0.3, hi_y=0.3), 1.0, 3e-2, 6)
+        assert 1 <= aw.aw_trig_level(ens, dt) <= 7
+        ens.flavour = flavour
+        aw.aw_integrate(ens, n, 400, dt, 100)
+        res.append(ens)
+    for other in res[1:]:
+        assert torch.equal(res[0].q, other.q) and torch.equal(res[0].acc, other.acc)
+        assert torch.equal(res[0].wind, other.wind) and torch.equal(res[0].status, other.status)
+        if tangent:
+            assert torch.equal(res[0].w, other.w)
+    res[0].flavour = 3
+    with pytest.raises(aw.AwError):
+        aw.aw_integrate(res[0], n, 100, dt, 100)
+
+
 # ------------------------------------------------------------------ odd histogram sizes, dropped points
 
 def test_odd_histogram_sizes_with_dropped_points(aw, orc):
