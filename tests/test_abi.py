@@ -181,6 +181,17 @@ def test_validation_happens_on_the_host(aw):
     assert lv(0.005) == 1 and block(32000, 0.2) == 64            # level 8: table kernel, 1000 blocks of 32 > 148 x 6
     assert block(28000, 0.2) == 32 and block(57000, 0.2) == 128   # 875 blocks fit; 891 blocks of 64 do not
     assert block(32000, 0.0628, order=6, E=15.0, eps=1.0) == 64   # the paper's Fig. 4 ensemble
+    # aw_kernel_schedule: latency flavour (0) up to 8 warps per sub-partition, throughput (1) beyond, where it exists
+    L.aw_kernel_schedule.argtypes = [C.POINTER(AwState), C.c_double]
+    def schedule(n, dt, flavour=0):
+        bs.n, bs.order, bs.E, bs.eps, bs.flavour = n, 4, 1.0, 3e-2, flavour
+        r = L.aw_kernel_schedule(C.byref(bs), dt)
+        bs.flavour = 0
+        return r
+    assert [schedule(n, 0.005) for n in (4096, 151552, 151553, 1 << 22)] == [0, 0, 1, 1]
+    assert schedule(1 << 22, 0.5) == 0 and schedule(1 << 22, 1.2) == 0          # levels 9 and 0: one flavour only
+    assert schedule(4096, 0.005, flavour=1) == 1 and schedule(1 << 22, 0.005, flavour=2) == 0
+    assert schedule(4096, 0.005, flavour=3) == EINVAL
     bs.block = 128
     assert block(5, 0.005) == 128
     bs.block = 0
