@@ -287,7 +287,7 @@ def _sampled_full_size(aw, orc, cfg, steps, ref=False):
     n = cfg["gx"] * cfg["gy"]
     ens = aw.Ensemble(n, tangent=cfg["tangent"], wind=True, order=cfg["order"], ref=ref)
     g = aw.make_grid(cfg["gx"], cfg["gy"], cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"], cfg["cx"],
-                     cfg["cy"], cfg["r"])
+                     cfg["cy"], cfg["r"], resample=cfg.get("resample", 0))
     aw.aw_init_shell(ens, g, cfg["E"], cfg["eps"], cfg["seed"])
     if ref:
         aw.aw_mark(ens)
@@ -369,12 +369,15 @@ def test_config4_full_cloud_parity_and_density(aw, orc):
     assert np.all(np.abs(got.acc[3, sample] - st0.acc[3, sample]) <= tol)
 
 
-def test_paper_workload_full_size_sampled_parity(aw, orc):
-    """configs 6 (the paper's Fig. 3a workload in its own units: E = 15, eps = 1, sixth order, h = 0.01 T, 2^22
-    initial conditions uniform on S x torus) in the launch configuration bench.py --config 6 times: state parity
-    on sampled trajectories after 100 steps, then the sphere density bit-exact on the device states."""
-    cfg = aw.CONFIGS[6]
+@pytest.mark.parametrize("cfgk", [5, 6, 8])
+def test_paper_workload_full_size_sampled_parity(aw, orc, cfgk):
+    """configs 5, 6 (the paper's Fig. 2a / 3a workloads in its own units: E = 400 / 15, eps = 1, sixth order, h = 0.01 T,
+    2^22 initial conditions uniform on S x torus) and 8 (the Fig. 4 cloud at W, 2^20 trajectories) in the launch
+    configuration bench.py --config K times (table-driven sincos at every stage for E = 400, mixed for E = 15): state
+    parity on sampled trajectories after 100 steps, then the sphere density bit-exact on the device states."""
+    cfg = aw.CONFIGS[cfgk]
     ens, st, got, sample = _sampled_full_size(aw, orc, cfg, 100, ref=True)
+    assert aw.aw_trig_level(ens, cfg["dt"]) == (9 if cfgk == 5 else 7) and aw.aw_kernel_schedule(ens, cfg["dt"]) == (0 if cfgk == 5 else 1)
     assert np.all(got.status == 1)
     err = state_rel_err(got.q[:, sample], got.wind[:, sample], st.q[:, sample], st.wind[:, sample],
                         np.ones(len(sample), bool))
@@ -387,10 +390,12 @@ def test_paper_workload_full_size_sampled_parity(aw, orc):
     h = hist.cpu().numpy().view(np.uint32)
     assert np.array_equal(h, ref) and int(dropped.item()) == int(d[0])
     assert int(h.sum()) + int(d[0]) == ens.n
-    # the projected points fill the disk |Vhat_xy| <= sqrt(2E) and nothing outside it
+    # the projected points lie in the disk |Vhat_xy| <= sqrt(2E); the sphere ensembles fill it
     yy, xx = np.mgrid[0:1024, 0:1024]
     r2 = ((xx + 0.5) / 512 - 1) ** 2 + ((yy + 0.5) / 512 - 1) ** 2
-    assert h[r2 > 1.01].sum() == 0 and (h[r2 < 0.9] > 0).mean() > 0.85
+    assert h[r2 > 1.01].sum() == 0
+    if cfgk != 8:
+        assert (h[r2 < 0.9] > 0).mean() > 0.85
 
 
 @pytest.mark.parametrize("cfgk,nsample", [(1, 32), (3, 32), (2, 16)])
