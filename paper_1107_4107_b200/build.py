@@ -30,13 +30,18 @@ def _nvcc():
 
 
 def source_hash():
-    """16 hex digits identifying what libaw.so is built from: every source, header and the compiler flags.  bench.py
-    quotes an ncu-measured DRAM traffic figure only when it was captured on the same build (profiles/traffic_by_build.csv)."""
+    """16 hex digits identifying what libaw.so is built from: every source and header with comments and blank
+    space removed (an edit that changes no code keeps the hash) and the compiler flags.  bench.py quotes an
+    ncu-measured DRAM traffic figure only when it was captured on the same build (profiles/traffic_by_build.csv)."""
     import hashlib
+    import re
     h = hashlib.sha256()
     for f in sorted(set(SOURCES + HEADERS)):
+        text = open(os.path.join(CSRC, f), encoding="utf-8").read()
+        text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)        # block comments
+        text = re.sub(r"//[^\n]*", " ", text)                     # line comments (no string literal here holds //)
         h.update(f.encode())
-        h.update(open(os.path.join(CSRC, f), "rb").read())
+        h.update(" ".join(text.split()).encode())
     h.update(repr((NVCC_FLAGS, UNITS)).encode())
     return h.hexdigest()[:16]
 

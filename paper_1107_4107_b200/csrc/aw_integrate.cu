@@ -13,27 +13,31 @@
 // (a_1 = a_{S+1} for the palindromic stage lists, so the last merged drift minus a_1 P is the closing drift).
 //
 // Model (eq. 2): H_p = cos x cos y (1 + cos 2z) = (cos u + cos v)(1 + cos zeta)/2 in the working
-// variables u = x + y, v = x - y, zeta = 2z the kernel holds inside a block (struct Traj below), so
+// variables u = x + y, v = x - y, zeta = 2z the kernel holds inside a block, every momentum-like variable doubled
+// (struct Traj below), so
 //   grad H_p = -(F sin u, F sin v, (cos u + cos v) sin zeta),  F = 1 + cos zeta   (d/du, d/dv, d/dz),
-// and the Hessian-vector product is the sum and difference of the x and y rows of SURVEY.md Appendix A.2.
+// and the Hessian-vector product is the sum and difference of the x and y rows of SURVEY.md Appendix A.2; with the
+// zeta pair carried scaled by 2 b_0 the kick of the first and last stage needs no constant multiplies (kick()).
 //
-// Trigonometry.  LEVEL 0: the table-driven sincos (tsincos below) of u, v, zeta at every stage.
-// LEVEL >= 1: the pairs (sin u, cos u), (sin v, cos v), (sin zeta, cos zeta) are carried in registers and
-// advanced through every drift by the rotation with the drift angle d = a p (p = pu, pv, pzeta):
+// Trigonometry, two mechanisms chosen per drift and per pair type at compile time from the LEVEL the
+// host picks (largest possible drift angle |d|) and the drift's ratio to the longest one:
+// (i) the pairs (sin u, cos u), (sin v, cos v), (sin zeta, cos zeta) are carried in registers and advanced through a
+// drift by the rotation with the drift angle d = A p:
 //     s' = s + (s m + c g),  c' = c + (c m - s g),   g = sin d = p G(p^2),  m = cos d - 1 = p^2 M(p^2),
-// G and M being the Taylor polynomials of sin and cos - 1 with the powers of a folded into their
-// coefficients on the host; the degree of every drift is fixed at compile time from the level the host picks
-// (largest possible |d|) and the drift's ratio to the largest one, so that the truncation error stays below
-// 2^-60 (rotation_degree, trig_level_for).  The pairs are re-synchronised from the tracked angles with the
-// full sincos after the opening drift of every block and at least every kMaxChunk steps, which bounds the
-// rounding random walk of the rotations at a few 1e-15.
+// G and M being the Taylor polynomials of sin and cos - 1 with the powers of A folded into their coefficients on the
+// host, of the smallest degree (<= 5) that keeps the truncation below 2^-60 (rotation_degree, trig_level_for).  A
+// pair type every drift rotates is re-synchronised from the tracked angle with the full sincos after the opening
+// drift of every block and at least every kMaxChunk steps, which bounds the rounding random walk of the rotations at
+// a few 1e-15.  (ii) After a drift too long for that, the kick evaluates the pair from the angle with the
+// table-driven sincos of aw_tsincos.cuh (LEVEL 0: at every stage).
 //
 // Instruction shapes (profiles/r1c_dfma_operand_shapes.md): on sm_100 a DFMA that reads three distinct 64-bit
 // registers issues every 3 cycles instead of 2 unless one operand comes from the operand-reuse cache, a
 // uniform register or an immediate, and every non-fp64 instruction takes an issue cycle the fp64 pipe also
 // needs.  The code below therefore minimises register reads and integer work, not just fp64 instructions:
 // coefficients and stage constants in uniform registers, the working variables above (16 three-register
-// multiply-adds per stage instead of 21), three-register FMAs written in groups that share an operand.
+// multiply-adds per stage instead of 21), three-register FMAs written in groups that share an operand, no quadrant
+// logic anywhere in the step loop.
 #include <cmath>
 
 #include "aw_internal.cuh"
@@ -44,9 +48,8 @@
 #ifndef AW_BLOCK
 #define AW_BLOCK 128
 #endif
-// Register cap: __launch_bounds__(128, 3) allows 168 registers per thread; the kernels take 102-134, which still
-// places 4 (order 6 without tangent at the high levels: 3) blocks per SM, and 3 warps per sub-partition already
-// saturate the fp64 pipe.  With the cap at 128 ptxas finds fewer operand-reuse pairs in most instantiations
+// Register cap: __launch_bounds__(128, 3) allows 168 registers per thread; the kernels take 94-144, which still
+// places 3-5 blocks per SM, and 3 warps per sub-partition already saturate the fp64 pipe.  With the cap at 128 ptxas finds fewer operand-reuse pairs in most instantiations
 // (measured: configs[3] -1.1 %), except the level-4 ones (configs[2]: +1.8 % at 128), which keep 4.
 #ifndef AW_MIN_BLOCKS
 #define AW_MIN_BLOCKS(LEVEL) ((LEVEL) == 4 ? 4 : 3)
