@@ -259,13 +259,14 @@ struct awo_grid {
   double lo_x, hi_x, lo_y, hi_y;
   int32_t angle_mode;    // 0: all angles 0; 1: U[0,2pi) from seed
   int32_t shape;         // 0: grid; 1: uniform disk (cx,cy,r); 2: Gaussian (cx,cy,sigma=r);
-                         // 3: uniform on the whole sphere S (R28)
+                         // 3: uniform on the whole sphere S (R28);
+                         // 4: uniform random points of the rectangle [lo_x,hi_x) x [lo_y,hi_y) (R33)
   double cx, cy, r;
   int32_t pz_sign;       // +1 or -1
   int32_t tangent_mode;  // 0: one common seeded unit vector; 1: per trajectory
   int64_t k0;            // the state holds trajectories [k0, k0 + n) of the gx*gy ensemble the grid describes
                          // (independent realisations, so any contiguous slice can be generated alone)
-  int32_t resample;      // cloud shapes 1, 2: redraw a trajectory whose (px, py, X) has no real v_z, up to this many
+  int32_t resample;      // random shapes 1, 2, 4: redraw a trajectory whose (px, py, X) has no real v_z, up to this many
                          // times (R31); 0: mask it (status 0, R8)
   int32_t reserved_;
 };
@@ -315,7 +316,7 @@ int awo_init_shell(const awo_grid *g, double E, double eps, uint64_t seed, int64
     // trajectory is drawn again — attempt a takes ALL its draws (angles and cloud point) from the seed
     // seed_a = seed + a * 0xD1B54A32D192ED03 (mod 2^64) — until it lies on the shell; the accepted points are
     // distributed exactly like the unmasked points of the plain ensemble (rejection sampling).
-    const int attempts = (g->shape == 1 || g->shape == 2) && g->resample > 0 ? g->resample + 1 : 1;
+    const int attempts = (g->shape == 1 || g->shape == 2 || g->shape == 4) && g->resample > 0 ? g->resample + 1 : 1;
     for (int a = 0; a < attempts; ++a) {
       const uint64_t sd = seed + (uint64_t)a * 0xD1B54A32D192ED03ull;
       double X[3] = {0.0, 0.0, 0.0};
@@ -340,6 +341,13 @@ int awo_init_shell(const awo_grid *g, double E, double eps, uint64_t seed, int64
         if (g->shape == 0) {
           px = g->lo_x + ((double)i + 0.5) * (g->hi_x - g->lo_x) / (double)g->gx;
           py = g->lo_y + ((double)j + 0.5) * (g->hi_y - g->lo_y) / (double)g->gy;
+        } else if (g->shape == 4) {
+          // P:87 "initial conditions uniformly distributed within a small segment of the sphere (enclosed by the two
+          // squares in Fig. 2 (a))": the segment is a square in the view of S along the third axis, i.e. a rectangle
+          // in (px, py), sampled uniformly at random (R33); v_z from the energy condition as for the clouds
+          const double u1 = uniform01(sd, (uint64_t)K, 3), u2 = uniform01(sd, (uint64_t)K, 4);
+          px = g->lo_x + u1 * (g->hi_x - g->lo_x);
+          py = g->lo_y + u2 * (g->hi_y - g->lo_y);
         } else {
           const double u1 = uniform01(sd, (uint64_t)K, 3), u2 = uniform01(sd, (uint64_t)K, 4);
           const double ang = TWO_PI_HI * u2;

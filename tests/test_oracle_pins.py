@@ -642,3 +642,32 @@ def test_cloud_resampling_is_rejection_sampling(orc):
         a_ = orc.init_shell(orc.State(64, tangent=False), orc.make_grid(8, 8, angle_mode=1, shape=shape, resample=0), 1.0, 3e-2, 1)
         b_ = orc.init_shell(orc.State(64, tangent=False), orc.make_grid(8, 8, angle_mode=1, shape=shape, resample=9), 1.0, 3e-2, 1)
         assert np.array_equal(a_.q, b_.q, equal_nan=True)
+
+
+def test_random_rectangle_patch(orc):
+    """R33 (P:87 "uniformly distributed within a small segment of the sphere (enclosed by the two squares ...)"):
+    shape 4 draws (px, py) uniformly at random in [lo_x, hi_x) x [lo_y, hi_y): px = lo_x + u3 (hi_x - lo_x) with the
+    generator's own draws (retyped here), uniform by chi-square, v_z from the energy condition, angles uniform."""
+    n = 1 << 14
+    lo_x, hi_x, lo_y, hi_y = 1.0, 1.5, -2.25, -2.0
+    g = orc.make_grid(128, 128, lo_x, hi_x, angle_mode=1, shape=4, lo_y=lo_y, hi_y=hi_y)
+    st = orc.init_shell(orc.State(n, tangent=False), g, 15.0, 1.0, 21)
+    assert np.all(st.status == 1)                                   # well inside the E = 15 shell: P^2 <= 7.3 < 26
+    u3 = np.array([orc.uniform(21, k, 3) for k in range(n)])
+    u4 = np.array([orc.uniform(21, k, 4) for k in range(n)])
+    assert np.array_equal(st.q[3, :n], lo_x + u3 * (hi_x - lo_x)) and np.array_equal(st.q[4, :n], lo_y + u4 * (hi_y - lo_y))
+    assert st.q[3, :n].min() >= lo_x and st.q[3, :n].max() < hi_x and st.q[4, :n].min() >= lo_y and st.q[4, :n].max() < hi_y
+    counts = np.histogram2d(st.q[3, :n], st.q[4, :n], bins=8, range=((lo_x, hi_x), (lo_y, hi_y)))[0].ravel()
+    assert ((counts - n / 64) ** 2 / (n / 64)).sum() < 120          # 63 dof: mean 63, sd 11
+    assert abs(np.corrcoef(st.q[3, :n], st.q[4, :n])[0, 1]) < 0.03
+    H = 0.5 * (st.q[3:, :n] ** 2).sum(0) + np.cos(st.q[0, :n]) * np.cos(st.q[1, :n]) * (1 + np.cos(2 * st.q[2, :n]))
+    assert np.max(np.abs(H - 15.0)) < 64 * np.spacing(15.0) and np.all(st.q[5, :n] > 0)
+    # a patch that reaches over the edge of the shell: masked, or drawn again with resample (R31)
+    g2 = orc.make_grid(64, 64, 3.6, 4.0, angle_mode=1, shape=4, lo_y=3.6, hi_y=4.0)
+    s2 = orc.init_shell(orc.State(4096, tangent=False), g2, 15.0, 1.0, 21)
+    assert 0 < (s2.status == 0).sum() < 4096
+    g3 = orc.make_grid(64, 64, 3.6, 4.0, angle_mode=1, shape=4, lo_y=3.6, hi_y=4.0, resample=60)
+    s3 = orc.init_shell(orc.State(4096, tangent=False), g3, 15.0, 1.0, 21)
+    assert np.all(s3.status == 1)
+    first = s2.status == 1
+    assert np.array_equal(s3.q[:, :4096][:, first], s2.q[:, :4096][:, first])
