@@ -135,6 +135,9 @@ def workload_config(cfg, order, tangent, horizon, world, scaling, live_all):
                  % (n_rank * (16 * 8 + 12 + 1) / 1e6) if n_rank * 141 > 126e6 else
                  "state planes %.1f MB per rank; a 256 MB buffer is written between timed passes to flush L2"
                  % (n_rank * (16 * 8 + 12 + 1) / 1e6)}
+    if cfg.get("survive"):
+        out["survivors"] = ("survivor filter on the launch square (P:99): live_trajectories counts the survivors at the end; "
+                            "trajectories that left stopped being integrated, so `value` undercounts the work done")
     if cfg.get("window"):
         out["window_steps"] = cfg["window"]
     if cfg.get("density_every"):
@@ -320,6 +323,8 @@ def run_ours(args, cfg, order, tangent):
         aw.aw_init_shell(ens, grid, cfg["E"], cfg["eps"], cfg["seed"])
         hist.zero_()
         dropped.zero_()
+        if cfg.get("survive"):                       # only trajectories that stay inside the launch square
+            ens.set_survivors((cfg["lo"], cfg["hi"], cfg["lo"], cfg["hi"]))
         if dens_mode and not window:
             aw.aw_mark(ens)                          # X(t) of the averaging window
         if record:

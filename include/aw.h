@@ -57,7 +57,7 @@ enum { AW_IND_FLI = 0, AW_IND_FTLE = 1, AW_IND_DH = 2, AW_IND_CLASS = 3,
 /* aw_density modes: instantaneous actions (BASELINE) or the paper's projected averaged velocity (R19, R26) */
 enum { AW_DENS_ACTION = 0, AW_DENS_VEL_UPPER = 1, AW_DENS_VEL_LOWER = 2, AW_DENS_VEL_BOTH = 3 };
 /* aw_grid.shape */
-enum { AW_SHAPE_GRID = 0, AW_SHAPE_DISK = 1, AW_SHAPE_GAUSS = 2, AW_SHAPE_SPHERE = 3 };
+enum { AW_SHAPE_GRID = 0, AW_SHAPE_DISK = 1, AW_SHAPE_GAUSS = 2, AW_SHAPE_SPHERE = 3, AW_SHAPE_RECT = 4 };
 /* per-trajectory status byte */
 enum { AW_ST_OFFSHELL = 0, AW_ST_LIVE = 1, AW_ST_NONFINITE = 2, AW_ST_LEFT = 3,
        AW_ST_RANGE = 4 /* energy above the bound aw_integrate was launched for (see aw_state.Emax): not integrated */ };
@@ -123,7 +123,10 @@ typedef struct {
                                                SPHERE (R28) direction uniform on the unit sphere:
                                                  cos(th) = 1 - 2 u3, phi = 2pi u4, |P| = sqrt(2(E - eps H_p(X)))
                                                  P = |P| (sin th cos phi, sin th sin phi, pz_sign cos th);
-                                                 never off the shell; lo/hi/cx/cy/r unused        */
+                                                 never off the shell; lo/hi/cx/cy/r unused
+                                               RECT ("a small segment of the sphere"; R33) uniform random
+                                                 points of the rectangle: px = lo_x + u3 (hi_x - lo_x),
+                                                 py = lo_y + u4 (hi_y - lo_y)                     */
   double cx, cy, r;
   int32_t pz_sign;              /* +1 (default, upper hemisphere; R9) or -1                    */
   int32_t tangent_mode;         /* 0: one common seeded unit vector (R12); 1: per trajectory   */
@@ -131,7 +134,7 @@ typedef struct {
                                    position and every random draw are functions of the GLOBAL index K, so a slice
                                    is bit-identical to the same rows of the whole (multi-GPU sharding, P:13, P:63;
                                    R30): rank r of a row-sharded job passes k0 = j0*gx, n = rows*gx          */
-  int32_t resample;             /* shapes DISK, GAUSS: a draw (px, py, X) with 2(E - eps H_p(X)) < px^2 + py^2 has no
+  int32_t resample;             /* shapes DISK, GAUSS, RECT: a draw (px, py, X) with 2(E - eps H_p(X)) < px^2 + py^2 has no
                                    real third action ("v_z from the fixed energy condition").  0: mask it (status
                                    0, R8).  m > 0: draw the trajectory again, up to m times — attempt a takes ALL its
                                    draws (angles, cloud point) from seed_a = seed + a*0xD1B54A32D192ED03 (mod 2^64) —

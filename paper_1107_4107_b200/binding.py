@@ -16,7 +16,7 @@ AW_OK, AW_EINVAL, AW_ECUDA, AW_ERANGE, AW_ESTATE = 0, -1, -2, -3, -4
 AW_IND_FLI, AW_IND_FTLE, AW_IND_DH, AW_IND_CLASS = 0, 1, 2, 3
 AW_IND_DP, AW_IND_VX, AW_IND_VY, AW_IND_VZ, AW_IND_DHS = 4, 5, 6, 7, 8
 AW_DENS_ACTION, AW_DENS_VEL_UPPER, AW_DENS_VEL_LOWER, AW_DENS_VEL_BOTH = 0, 1, 2, 3
-AW_SHAPE_GRID, AW_SHAPE_DISK, AW_SHAPE_GAUSS, AW_SHAPE_SPHERE = 0, 1, 2, 3
+AW_SHAPE_GRID, AW_SHAPE_DISK, AW_SHAPE_GAUSS, AW_SHAPE_SPHERE, AW_SHAPE_RECT = 0, 1, 2, 3, 4
 AW_ST_OFFSHELL, AW_ST_LIVE, AW_ST_NONFINITE, AW_ST_LEFT, AW_ST_RANGE = 0, 1, 2, 3, 4
 
 

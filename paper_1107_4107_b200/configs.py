@@ -51,6 +51,15 @@ CONFIGS = {
             cx=3.872983346207417, cy=3.872983346207417, r=0.01, E=15.0, eps=1.0, seed=2011, order=6,
             dt=0.06283185307179587, steps=20_000, stride=100, tangent=False, density_every=0, density_mode=3,
             window=5_000, resample=40, hist_lo=-5.477225575051661, hist_hi=5.477225575051661),
+    # The paper's zooms (Figs. 2b,c / 3b,c): initial conditions uniformly distributed at random within a
+    # small square segment of the sphere (seen along the third axis: a square in (px, py), R33), uniform torus angles,
+    # v_z from the energy condition; "tracked only those trajectories which remained within the area during the whole
+    # observation time" (survivor filter on the launch square, R25); averaging interval doubled to Dt = 100 T as for the
+    # highest resolution (Fig. 3c); density of the projected averaged velocity over the same square.  The square
+    # sits on the resonance plane px = py (Omega_(1,-1,0)) of the E = 15 shell; the paper does not print its own.
+    9: dict(name="paper_fig3c_zoom_E15_square_survivors", gx=2048, gy=2048, lo=2.0, hi=2.5, angle_mode=1, shape=4,
+            cx=0.0, cy=0.0, r=0.0, E=15.0, eps=1.0, seed=2011, order=6, dt=0.06283185307179587, steps=10_000,
+            stride=100, tangent=False, density_every=0, density_mode=3, survive=True, hist_lo=2.0, hist_hi=2.5),
 }
 
 HIST_G = 1024          # density histogram is HIST_G x HIST_G over [HIST_LO, HIST_HI]^2 (configs[4])

@@ -289,7 +289,7 @@ int aw_init_shell(aw_state *s, const aw_grid *grid, double E, double eps, uint64
   if (grid->angle_mode != 0 && grid->angle_mode != 1) return AW_EINVAL;
   if (grid->tangent_mode != 0 && grid->tangent_mode != 1) return AW_EINVAL;
   if (grid->resample < 0 || grid->resample > 1024) return AW_EINVAL;
-  if (grid->shape == AW_SHAPE_GRID) {
+  if (grid->shape == AW_SHAPE_GRID || grid->shape == AW_SHAPE_RECT) {
     if (!(grid->hi_x > grid->lo_x) || !(grid->hi_y > grid->lo_y)) return AW_EINVAL;
     if (!std::isfinite(grid->lo_x) || !std::isfinite(grid->hi_x) || !std::isfinite(grid->lo_y) ||
         !std::isfinite(grid->hi_y))

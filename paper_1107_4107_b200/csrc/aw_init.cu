@@ -38,7 +38,8 @@ __global__ void __launch_bounds__(256) init_shell_kernel(const __grid_constant__
   double x = 0.0, y = 0.0, z = 0.0, px = nan, py = nan, pz = nan, H0 = nan;
   bool live = false;
   // cloud shapes with resample > 0: draw again until the point has a real third action (R31; include/aw.h)
-  const int attempts = (g.shape == AW_SHAPE_DISK || g.shape == AW_SHAPE_GAUSS) && g.resample > 0 ? g.resample + 1 : 1;
+  const int attempts =
+      (g.shape == AW_SHAPE_DISK || g.shape == AW_SHAPE_GAUSS || g.shape == AW_SHAPE_RECT) && g.resample > 0 ? g.resample + 1 : 1;
   for (int a = 0; a < attempts && !live; ++a) {
     const uint64_t sd = p.seed + (uint64_t)a * 0xD1B54A32D192ED03ull;
     if (g.angle_mode == 1) {
@@ -62,6 +63,11 @@ __global__ void __launch_bounds__(256) init_shell_kernel(const __grid_constant__
       if (g.shape == AW_SHAPE_GRID) {
         px = __dadd_rn(g.lo_x, __ddiv_rn(__dmul_rn(__dadd_rn((double)i, 0.5), __dsub_rn(g.hi_x, g.lo_x)), (double)g.gx));
         py = __dadd_rn(g.lo_y, __ddiv_rn(__dmul_rn(__dadd_rn((double)j, 0.5), __dsub_rn(g.hi_y, g.lo_y)), (double)g.gy));
+      } else if (g.shape == AW_SHAPE_RECT) {
+        // uniform random points of a rectangle in (px, py) (R33)
+        const double u1 = uniform01(sd, uk, 3), u2 = uniform01(sd, uk, 4);
+        px = __dadd_rn(g.lo_x, __dmul_rn(u1, __dsub_rn(g.hi_x, g.lo_x)));
+        py = __dadd_rn(g.lo_y, __dmul_rn(u2, __dsub_rn(g.hi_y, g.lo_y)));
       } else {
         const double u1 = uniform01(sd, uk, 3), u2 = uniform01(sd, uk, 4);
         const double rad = (g.shape == AW_SHAPE_DISK) ? __dmul_rn(g.r, sqrt(u1))

@@ -148,6 +148,55 @@ def test_cloud_resampling_matches_oracle_generator(aw, orc, shape, resample):
         aw.aw_init_shell(ens, bad, 15.0, 1.0, 31)
 
 
+# ------------------------------------------------------------------ P:87 / P:99: random square segment, survivors
+
+def test_zoom_square_with_survivors_parity(aw, orc):
+    """CONFIGS[9] at reduced size: initial conditions uniformly at random in a square segment of the sphere (shape
+    RECT), survivor filter on the launch square, window Dt = 100 T.  Generator bit-equal to the
+    oracle's (px, py are hash * constant arithmetic); after 100 steps every state within 1e-10; after the window the
+    survivor statuses equal the oracle's except where (px, py) passes within rounding distance of an edge, and the
+    sphere density of the survivors is bit-exact on the device states."""
+    cfg = aw.CONFIGS[9]
+    gx, gy = 96, 64
+    n = gx * gy
+    rect = (cfg["lo"], cfg["hi"], cfg["lo"], cfg["hi"])
+    mk = lambda mod: mod.make_grid(gx, gy, cfg["lo"], cfg["hi"], cfg["angle_mode"], cfg["shape"])
+    ens = aw.Ensemble(n, tangent=False, wind=True, order=cfg["order"], ref=True)
+    aw.aw_init_shell(ens, mk(aw), cfg["E"], cfg["eps"], cfg["seed"])
+    gen = orc.init_shell(orc.State(n, tangent=False), mk(orc), cfg["E"], cfg["eps"], cfg["seed"])
+    st = ensemble_to_oracle(ens, orc)
+    assert np.all(st.status == 1) and np.array_equal(st.status, gen.status)
+    assert np.array_equal(st.q[:5, :n], gen.q[:5, :n])                        # angles, px, py: bit-equal
+    assert np.max(np.abs(st.q[5, :n] - gen.q[5, :n])) <= 4e-15 * math.sqrt(34.0)
+    ens.set_survivors(rect)
+    aw.aw_mark(ens)
+    st = ensemble_to_oracle(ens, orc)
+    aw.aw_integrate(ens, n, 100, cfg["dt"], cfg["stride"])
+    orc.integrate(st, 100, cfg["dt"], cfg["stride"])
+    got = ensemble_to_oracle(ens, orc)
+    assert np.array_equal(got.status, st.status)
+    err = state_rel_err(got.q[:, :n], got.wind[:, :n], st.q[:, :n], st.wind[:, :n], np.ones(n, bool))
+    assert err.max() <= 1e-10, err.max()
+    aw.aw_integrate(ens, n, cfg["steps"] - 100, cfg["dt"], cfg["stride"])
+    oracle_integrate_mt(orc, st, cfg["steps"] - 100, cfg["dt"], cfg["stride"])
+    got = ensemble_to_oracle(ens, orc)
+    gone = st.status == 3
+    assert 0.2 * n < gone.sum() < n                                            # a chaotic neighbourhood: many leave
+    # decisions differ only for trajectories that graze an edge of the square (chaotic orbits decorrelate over 100 T)
+    assert (got.status != st.status).sum() <= 0.02 * n
+    assert abs((ens.t - ens.tref) - 100 * 2 * math.pi) < 1e-8
+    G = 128
+    hist = torch.zeros((G, G), dtype=torch.int32, device="cuda")
+    dropped = torch.zeros(1, dtype=torch.int64, device="cuda")
+    aw.aw_density(ens, hist, cfg["hist_lo"], cfg["hist_hi"], cfg["density_mode"], dropped)
+    ref = np.zeros((G, G), dtype=np.uint32)
+    d = orc.density_velocity(got, ref, cfg["hist_lo"], cfg["hist_hi"], cfg["density_mode"])
+    h = hist.cpu().numpy().view(np.uint32)
+    assert np.array_equal(h, ref) and int(dropped.item()) == int(d[0])
+    assert int(h.sum()) + int(d[0]) == int((got.status == 1).sum())
+    assert h.sum() > 0
+
+
 # ------------------------------------------------------------------ P:97 Fig. 4: consecutive windows
 
 def test_fig4_consecutive_windows_density_parity(aw, orc):
