@@ -75,3 +75,30 @@ def test_two_ranks_on_one_gpu_equal_the_single_process_result(tmp_path, case, sc
     img, hist = np.load(tmp_path / "img.npy"), np.load(tmp_path / "hist.npy")
     assert np.array_equal(img, ref_img.numpy(), equal_nan=True)
     assert np.array_equal(hist, ref_hist.numpy()) and hist.sum() > 0
+
+
+def _nccl_worker(rank, world, port, out_dir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", 0))
+    from paper_1107_4107_b200 import parallel
+    parallel._active = lambda: True                        # a world of one still goes through the collectives
+    hist = torch.arange(-8, 8, dtype=torch.int32, device="cuda").reshape(4, 4).contiguous()
+    before = hist.clone()
+    parallel.allreduce_hist(hist)
+    img = parallel.gather_image(torch.arange(5, dtype=torch.float64, device="cuda"), [5])
+    ok = torch.equal(hist, before) and img.is_cuda and torch.equal(img.cpu(), torch.arange(5, dtype=torch.float64))
+    cls = parallel.gather_image(torch.arange(7, dtype=torch.uint8, device="cuda"), [7])     # CLASS images are bytes
+    ok = ok and torch.equal(cls.cpu(), torch.arange(7, dtype=torch.uint8))
+    open(os.path.join(out_dir, "ok"), "w").write(str(bool(ok)))
+    dist.destroy_process_group()
+
+
+def test_nccl_collectives_on_device_tensors(tmp_path):
+    """bench.py's N > 1 path calls NCCL all_reduce on the int32 histogram and NCCL gather on the fp64 (or uint8) image
+    where they live, on the device.  With one GPU the communicator has one rank; this checks that the calls are the
+    ones NCCL accepts for these dtypes and shapes (the exchange itself is trivial)."""
+    assert torch.cuda.is_available()
+    mp.spawn(_nccl_worker, args=(1, _free_port(), str(tmp_path)), nprocs=1, join=True)
+    assert open(tmp_path / "ok").read() == "True"
