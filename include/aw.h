@@ -269,8 +269,7 @@ AW_API int aw_trig_level(const aw_state *s, double dt);
  * of aw_integrate does not depend on it.  Negative aw_status as aw_trig_level. */
 AW_API int aw_block_size(const aw_state *s, double dt);
 /* Which ptxas schedule of the integrator kernel aw_integrate launches for this state and dt (aw_state.flavour): 1 = the
- * throughput flavour, 0 = the latency flavour (always 0 for the levels that exist in one flavour only: 0, 8, 9); or a
- * negative aw_status.  The kernel is integrate_kernel<S, TAN, LEVEL, SCHEDULE> with S = 3 / 7 stages. */
+ * throughput flavour, 0 = the latency flavour; or a negative aw_status.  The kernel is integrate_kernel<S, TAN, LEVEL, SCHEDULE> with S = 3 / 7 stages. */
 AW_API int aw_kernel_schedule(const aw_state *s, double dt);
 /* The common tangent vector of tangent_mode 0: unit vector from u(seed, 2^63-1, 5..10) (R12). */
 AW_API int aw_common_tangent(uint64_t seed, double *t6_host);

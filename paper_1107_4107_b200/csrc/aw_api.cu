@@ -271,7 +271,7 @@ int aw_kernel_schedule(const aw_state *s, double dt) {
   if (!s || s->n < 0 || s->flavour < 0 || s->flavour > 2) return AW_EINVAL;
   const int level = aw_trig_level(s, dt);
   if (level < 0) return level;
-  return (level >= 1 && level <= 7 && !integrate_latency_flavour(s->n, s->flavour)) ? 1 : 0;
+  return integrate_latency_flavour(s->n, s->flavour) ? 0 : 1;
 }
 
 int aw_common_tangent(uint64_t seed, double *t6_host) {

@@ -56,17 +56,16 @@
 #endif
 
 // This file is compiled twice (build.py), the same source and the same arithmetic under two ptxas schedules:
-//   AW_LEVEL_GROUP 1, -Xptxas -O1, trig levels 1-7: the lighter scheduler stays close to source order, which keeps the
-//     three-register FMAs that share an operand next to each other, so more of them hit the operand-reuse cache
-//     (measured on B200: configs[3] +3.5 %, configs[2] +3.5 %, order 6 +2.9 %), and needs fewer registers.  This is
-//     the THROUGHPUT flavour: best when the fp64 pipe is saturated (>= 3 warps per sub-partition).
-//   AW_LEVEL_GROUP 0, default flags, every level: ptxas interleaves the independent chains of a stage (the three pairs'
-//     polynomials, the three table look-ups), which is what a warp needs when it has a sub-partition almost to itself.
-//     This is the LATENCY flavour, used for small ensembles (the paper's Fig. 4 ensemble, 32 000 trajectories = 1.7
-//     warps per sub-partition: 2.94e10 -> 3.56e10 traj-steps/s; configs[0], 4096 trajectories: 1.46e10 -> 2.28e10;
-//     the same kernels on 6e5 trajectories: -1 to -3 %), and the
-//     only one for the levels whose step loop is dominated by the table sincos (0, 8, 9: -3 % at -O1).  It also holds
-//     the host-side functions.
+//   AW_LEVEL_GROUP 1, -Xptxas -O1: the lighter scheduler stays close to source order, which keeps the three-register
+//     FMAs that share an operand next to each other, so more of them hit the operand-reuse cache (measured on B200:
+//     configs[3] +3.5 %, configs[2] +3.5 %, order 6 +2.9 %; the table kernel of the E = 400 workload +1.9 %), and needs
+//     fewer registers.  This is the THROUGHPUT flavour: best when the fp64 pipe is saturated (>= 3 warps per
+//     sub-partition).
+//   AW_LEVEL_GROUP 0, default flags: ptxas interleaves the independent chains of a stage (the three pairs' polynomials,
+//     the three table look-ups), which is what a warp needs when it has a sub-partition almost to itself.  This is the
+//     LATENCY flavour, used for small ensembles (the paper's Fig. 4 ensemble, 32 000 trajectories = 1.7 warps per
+//     sub-partition: 2.94e10 -> 3.56e10 traj-steps/s; configs[0], 4096 trajectories: 1.46e10 -> 2.28e10; the same
+//     kernels on 6e5 trajectories: -1 to -3 %).  It also holds the host-side functions.
 // ptxas does not reassociate floating-point arithmetic, so both flavours give the same bits (tested).
 #ifndef AW_LEVEL_GROUP
 #define AW_LEVEL_GROUP 0
@@ -451,8 +450,11 @@ cudaError_t launch_level(const IntegrateParams &p, cudaStream_t st) {
     case 5: return launch_one<S, TAN, 5>(p, st);
     case 6: return launch_one<S, TAN, 6>(p, st);
     case 7: return launch_one<S, TAN, 7>(p, st);
+    case 8: return launch_one<S, TAN, 8>(p, st);
+    case 9: return launch_one<S, TAN, 9>(p, st);
+    case 0: return launch_one<S, TAN, 0>(p, st);
     default: return cudaErrorInvalidValue;
-#else
+#else  // the latency flavour: every level
     case 1: return launch_one<S, TAN, 1>(p, st);
     case 2: return launch_one<S, TAN, 2>(p, st);
     case 3: return launch_one<S, TAN, 3>(p, st);
@@ -560,7 +562,7 @@ bool drift_ratios_hold(int S, const double *a_loop) {
 cudaError_t launch_integrate_low(const IntegrateParams &p, int order, bool tangent, cudaStream_t st);
 
 cudaError_t launch_integrate(const IntegrateParams &p, int order, bool tangent, bool latency, cudaStream_t st) {
-  if (p.level >= 1 && p.level <= 7 && !latency) return launch_integrate_low(p, order, tangent, st);
+  if (!latency) return launch_integrate_low(p, order, tangent, st);
   if (order == 4) return tangent ? launch_level<3, true>(p, st) : launch_level<3, false>(p, st);
   return tangent ? launch_level<7, true>(p, st) : launch_level<7, false>(p, st);
 }

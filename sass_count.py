@@ -28,9 +28,9 @@ def _functions(lib):
 
 def integrate_step_mix(order, tangent, level, lib=LIB, schedule=None):
     """{'dfma', 'dmul', 'dadd', 'other', 'flops'} per trajectory-step of integrate_kernel<S,TAN,LEVEL,SCHEDULE>.
-    schedule: 1 = the throughput flavour (levels 1-7 only), 0 = the latency flavour; None = 1 where it exists."""
+    schedule: 1 = the throughput flavour (default), 0 = the latency flavour."""
     if schedule is None:
-        schedule = 1 if 1 <= level <= 7 else 0
+        schedule = 1
     key = (os.path.getmtime(lib), order, bool(tangent), level, schedule)
     if key in _cache:
         return _cache[key]
@@ -88,6 +88,6 @@ if __name__ == "__main__":
     for order in (4, 6):
         for tangent in (False, True):
             for level in range(10):
-                for schedule in ((1, 0) if 1 <= level <= 7 else (0,)):
+                for schedule in (1, 0):
                     print(order, tangent, level, "throughput" if schedule else "latency   ",
                           integrate_step_mix(order, tangent, level, schedule=schedule))

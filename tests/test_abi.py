@@ -189,7 +189,7 @@ def test_validation_happens_on_the_host(aw):
         bs.flavour = 0
         return r
     assert [schedule(n, 0.005) for n in (4096, 151552, 151553, 1 << 22)] == [0, 0, 1, 1]
-    assert schedule(1 << 22, 0.5) == 0 and schedule(1 << 22, 1.2) == 0          # levels 9 and 0: one flavour only
+    assert schedule(1 << 22, 0.5) == 1 and schedule(4096, 1.2) == 0             # every level exists in both
     assert schedule(4096, 0.005, flavour=1) == 1 and schedule(1 << 22, 0.005, flavour=2) == 0
     assert schedule(4096, 0.005, flavour=3) == EINVAL
     bs.block = 128

@@ -485,16 +485,16 @@ def test_block_size_does_not_change_the_result(aw, order, tangent, dt):
 
 
 @pytest.mark.parametrize("order,tangent,dt", [(4, True, 0.005), (4, True, 0.025), (6, True, 0.02), (6, False, 0.0628),
-                                              (4, False, 0.1), (6, True, 0.15)])
+                                              (4, False, 0.1), (6, True, 0.15), (4, True, 0.2), (6, False, 1.0),
+                                              (4, True, 1.2)])
 def test_kernel_flavours_give_the_same_bits(aw, order, tangent, dt):
-    """Trig levels 1-7 exist in two ptxas schedules of the same source (throughput: source order for operand reuse;
+    """Every kernel exists in two ptxas schedules of the same source (throughput: source order for operand reuse;
     latency: interleaved chains for small ensembles); aw_integrate picks one from n.  Same arithmetic, same bits."""
     n = 3000 + 11
     res = []
     for flavour in (0, 1, 2):
         ens = aw.Ensemble(n, tangent=tangent, wind=True, order=order)
         aw.aw_init_shell(ens, aw.make_grid(n, 1, -0.9, 0.9, angle_mode=1, lo_y=-0.3, hi_y=0.3), 1.0, 3e-2, 6)
-        assert 1 <= aw.aw_trig_level(ens, dt) <= 7
         ens.flavour = flavour
         aw.aw_integrate(ens, n, 400, dt, 100)
         res.append(ens)
