@@ -377,7 +377,7 @@ def test_paper_workload_full_size_sampled_parity(aw, orc, cfgk):
     parity on sampled trajectories after 100 steps, then the sphere density bit-exact on the device states."""
     cfg = aw.CONFIGS[cfgk]
     ens, st, got, sample = _sampled_full_size(aw, orc, cfg, 100, ref=True)
-    assert aw.aw_trig_level(ens, cfg["dt"]) == (9 if cfgk == 5 else 7) and aw.aw_kernel_schedule(ens, cfg["dt"]) == (0 if cfgk == 5 else 1)
+    assert aw.aw_trig_level(ens, cfg["dt"]) == (9 if cfgk == 5 else 7) and aw.aw_kernel_schedule(ens, cfg["dt"]) == 1
     assert np.all(got.status == 1)
     err = state_rel_err(got.q[:, sample], got.wind[:, sample], st.q[:, sample], st.wind[:, sample],
                         np.ones(len(sample), bool))
