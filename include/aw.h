@@ -227,6 +227,20 @@ AW_API int aw_indicator(const aw_state *s, int kind, double thr, void *out_dev);
 AW_API size_t aw_energy_stats_scratch_bytes(int64_t n);
 AW_API int aw_energy_stats(const aw_state *s, void *scratch_dev, double *out_dev);
 
+/* aw_energy_stats for callers that cannot allocate device memory (under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): same kernels, same result bit for bit, but the block partials live in a static device
+ * array inside the library (AW_NOALLOC_MAX_N / 2048 partials of 64 bytes = 512 KiB, held by every GPU that loads the
+ * library until the process exits), so the caller passes only the state and out_dev (8 doubles, device, 16-byte
+ * aligned).  The call allocates and frees nothing: no cudaMalloc / cudaFree, no allocating library routine; the first
+ * call on a device looks the array's address up once (cudaGetSymbolAddress, with the current device — the one that
+ * holds s — current).  AW_ERANGE if s->n > AW_NOALLOC_MAX_N (use aw_energy_stats with caller scratch instead);
+ * otherwise the errors of aw_energy_stats.  Nothing in the array has to be cleared between calls (partials [0, nb)
+ * are overwritten before they are read) and a call never sees the previous call's contents.  All calls on one device
+ * SHARE the array: calls whose kernels can overlap on the GPU (different streams, no ordering between them) race —
+ * order them on one stream or with events.  Asynchronous on s->stream like aw_energy_stats. */
+#define AW_NOALLOC_MAX_N 16777216 /* 2^24 trajectories */
+AW_API int aw_energy_stats_noalloc(const aw_state *s, double *out_dev);
+
 /* §8(a) a6 — visited-cell density over the first two actions (R19, R20).  For each live
  * trajectory ix = floor((px - lo) * (gx/(hi - lo))), iy likewise with gy; inside -> hist[iy*gx + ix]
  * += 1, else *dropped_dev += 1 (dropped_dev may be NULL; 8-byte aligned).  ADDS into hist_dev (device, gx*gy

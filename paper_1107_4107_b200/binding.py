@@ -18,6 +18,7 @@ AW_IND_DP, AW_IND_VX, AW_IND_VY, AW_IND_VZ, AW_IND_DHS = 4, 5, 6, 7, 8
 AW_DENS_ACTION, AW_DENS_VEL_UPPER, AW_DENS_VEL_LOWER, AW_DENS_VEL_BOTH = 0, 1, 2, 3
 AW_SHAPE_GRID, AW_SHAPE_DISK, AW_SHAPE_GAUSS, AW_SHAPE_SPHERE, AW_SHAPE_RECT = 0, 1, 2, 3, 4
 AW_ST_OFFSHELL, AW_ST_LIVE, AW_ST_NONFINITE, AW_ST_LEFT, AW_ST_RANGE = 0, 1, 2, 3, 4
+AW_NOALLOC_MAX_N = 1 << 24      # aw_energy_stats_noalloc: size of the library's static scratch (include/aw.h)
 
 
 class AwError(RuntimeError):
@@ -94,6 +95,7 @@ def lib():
         L.aw_energy_stats_scratch_bytes.restype = C.c_size_t
         L.aw_energy_stats_scratch_bytes.argtypes = [i64]
         L.aw_energy_stats.argtypes = [C.POINTER(AwState), vp, vp]
+        L.aw_energy_stats_noalloc.argtypes = [C.POINTER(AwState), vp]
         L.aw_indicator.argtypes = [C.POINTER(AwState), C.c_int, dbl, vp]
         L.aw_density.argtypes = [C.POINTER(AwState), vp, i32, i32, dbl, dbl, C.c_int, vp]
         L.aw_stage_constants.argtypes = [C.c_int, dbl, dbl, C.POINTER(dbl), C.POINTER(dbl)]
@@ -305,6 +307,15 @@ def aw_energy_stats(ens, out=None, stream=None):
     if out is None:
         out = torch.empty((8,), dtype=torch.float64, device=ens.device)
     _check(lib().aw_energy_stats(C.byref(ens.c), _ptr(scratch), _ptr(out)), "aw_energy_stats")
+    return out
+
+
+def aw_energy_stats_noalloc(ens, out, stream=None):
+    """aw_energy_stats without any allocation: the scratch is a static device array inside libaw.so (at most
+    AW_NOALLOC_MAX_N trajectories); `out` is the caller's 8-double CUDA tensor.  Calls that overlap on the GPU race
+    on the shared scratch (include/aw.h)."""
+    ens.bind_stream(stream)
+    _check(lib().aw_energy_stats_noalloc(C.byref(ens.c), _ptr(out)), "aw_energy_stats_noalloc")
     return out
 
 

@@ -453,6 +453,18 @@ int aw_energy_stats(const aw_state *s, void *scratch_dev, double *out_dev) {
   return AW_OK;
 }
 
+int aw_energy_stats_noalloc(const aw_state *s, double *out_dev) {
+  if (!s || !out_dev) return AW_EINVAL;
+  int rc = check_planes(s);
+  if (rc != AW_OK) return rc;
+  if (!aligned16(out_dev)) return AW_EINVAL;
+  if (s->n > AW_NOALLOC_MAX_N) return AW_ERANGE;   // the static scratch array holds AW_NOALLOC_MAX_N / 2048 partials
+  if (!s->ready) return AW_ESTATE;
+  AW_CUDA(launch_energy_stats_noalloc(s->q, s->acc, s->status, s->n, s->pitch, s->eps, out_dev,
+                                      (cudaStream_t)s->stream));
+  return AW_OK;
+}
+
 int aw_density(const aw_state *s, uint32_t *hist_dev, int32_t gx, int32_t gy, double lo, double hi,
                int mode, uint64_t *dropped_dev) {
   if (!s || !hist_dev) return AW_EINVAL;

@@ -95,6 +95,10 @@ int64_t energy_stats_blocks(int64_t n);
 size_t energy_partial_bytes();
 cudaError_t launch_energy_stats(const double *q, const double *acc, const uint8_t *status, int64_t n, int64_t pitch,
                                 double eps, void *scratch, double *out, cudaStream_t st);
+// the same two kernels with the block partials in the library's own static device array (aw_energy_stats_noalloc)
+int64_t energy_stats_noalloc_max_n();
+cudaError_t launch_energy_stats_noalloc(const double *q, const double *acc, const uint8_t *status, int64_t n,
+                                        int64_t pitch, double eps, double *out, cudaStream_t st);
 cudaError_t launch_signed_dh(const double *q, const double *acc, const uint8_t *status, int64_t n, int64_t pitch,
                              double eps, double *out, cudaStream_t st);
 // max over live, finite trajectories of H(X,P), as a monotone 64-bit key (0 = none) in *key_out (aw_bound_energy)

@@ -1,5 +1,6 @@
 // aw_reduce.cu — §8(a) a5 (indicator image) and a6 (visited-cell density histogram); DESIGN.md §6.3-6.4.
 #include <cstring>
+#include <mutex>
 
 #include "aw_internal.cuh"
 #include "aw_model.cuh"
@@ -381,6 +382,57 @@ double energy_key_decode(unsigned long long key, bool *any) {
   static_assert(sizeof h == sizeof b, "fp64");
   memcpy(&h, &b, sizeof h);
   return h;
+}
+
+// ------------------------------------------------------------ aw_energy_stats_noalloc: scratch held by the library
+// The block partials of the energy statistics live in this file-scope device array instead of caller memory, so the
+// call needs no allocation from anybody (CUDA graph capture, serving loops).  Every device that loads the library
+// holds the 512 KiB until the process exits.  The name below is only a host-side handle in host code: the device
+// address is taken once per device with cudaGetSymbolAddress, with that device current, and handed to the kernels.
+// Nothing has to start at zero — energy_partial_kernel overwrites partials [0, nb) and energy_final_kernel reads
+// exactly those — so the previous call's contents are never seen.  All calls on a device share the array: two calls
+// whose kernels overlap on the GPU (different streams) race.
+constexpr int64_t kNoAllocMaxBlocks = (AW_NOALLOC_MAX_N + kStatsBlock * kStatsItems - 1) / (kStatsBlock * kStatsItems);
+static __device__ __align__(256) EnergyPartial g_noalloc_partials[kNoAllocMaxBlocks];
+
+namespace {
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+EnergyPartial *g_noalloc_addr[kNoAllocMaxDevices] = {};
+
+cudaError_t noalloc_scratch(EnergyPartial **out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kNoAllocMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_addr[dev]) {
+    void *p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_noalloc_partials);
+    if (e != cudaSuccess) return e;
+    g_noalloc_addr[dev] = static_cast<EnergyPartial *>(p);
+  }
+  *out = g_noalloc_addr[dev];
+  return cudaSuccess;
+}
+}  // namespace
+
+int64_t energy_stats_noalloc_max_n() { return kNoAllocMaxBlocks * kStatsBlock * kStatsItems; }
+
+cudaError_t launch_energy_stats_noalloc(const double *q, const double *acc, const uint8_t *status, int64_t n,
+                                        int64_t pitch, double eps, double *out, cudaStream_t st) {
+  EnergyPartial *part = nullptr;
+  const cudaError_t e = noalloc_scratch(&part);
+  if (e != cudaSuccess) return e;
+  const int64_t nb = energy_stats_blocks(n);
+  if (nb > kNoAllocMaxBlocks) return cudaErrorInvalidValue;   // the C entry rejects this before coming here
+  if (nb > 0) {
+    energy_partial_kernel<<<(unsigned)nb, kStatsBlock, 0, st>>>(q, acc, status, n, pitch, eps, part);
+    count_launch();
+  }
+  energy_final_kernel<<<1, kStatsBlock, 0, st>>>(part, nb, out);
+  count_launch();
+  return cudaGetLastError();
 }
 
 }  // namespace aw
