@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define AW_VERSION 200 /* 2.0.0: aw_grid.k0, aw_state.Emax / block, AW_ST_RANGE, aw_bound_energy; probes moved out */
+#define AW_VERSION 210 /* 2.1.0: + aw_energy_stats_noalloc.  2.0.0: aw_grid.k0, aw_state.Emax / block, AW_ST_RANGE, aw_bound_energy; probes out */
 
 #if defined(__GNUC__)
 #define AW_API __attribute__((visibility("default")))

@@ -31,7 +31,7 @@ def test_library_exports_every_declared_symbol(aw):
     L = C.CDLL(os.path.join(ROOT, "paper_1107_4107_b200", "libaw.so"))
     for n in names:
         assert hasattr(L, n), n
-    assert aw.aw_version() == 200
+    assert aw.aw_version() == 210
     assert not any("probe" in n for n in names)            # probes live in tests/libaw_probe.so, not in the product ABI
     assert aw.aw_strerror(0) == "ok" and "invalid" in aw.aw_strerror(-1)
 
